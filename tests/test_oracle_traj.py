@@ -1,0 +1,267 @@
+"""Pins for the oracle's time stepping (SSPRK(10,4) on the ray ODE of Eq.(22)).
+
+P5  pure 2-spin, quench T=inf -> T=0 (the exact case the paper uses for Fig.4):
+    textbook closed form (Cugliandolo-Dean), written here with scipy Bessel functions:
+      Gamma(t) = I1(4t)/(2t),  mu(t) = 2 I0(4t)/I1(4t) - 1/t,  E = -mu/2,
+      C(t,t') = [I1(2(t+t'))/(t+t')] / sqrt(Gamma(t)Gamma(t')),
+      R(t,t') = [I1(2 tau)/tau] sqrt(Gamma(t')/Gamma(t)),  tau = t-t'.
+P6  spherical constraint C(t,t)=1 and R(t,t^-)=1 along the run; causality is
+    structural (theta <= 1).
+P7  high-T paramagnet (BASELINE.json config 1): mu -> T + f'(1)/T, E -> -f(1)/T and the
+    equilibrium FDT  R = (1/T) dC/dt'  at late times.
+P8  brute force: uniform tensor grid C[i][j], R[i][j], trapezoid memory sums, Heun, Richardson
+    in dt -- a different discretisation of Eq.(1)/(13) written here from scratch.
+P9  SSPRK(10,4): order conditions of the Butcher tableau, embedded weights are order 3 and not 4,
+    the low-storage form equals the tableau form, 4th-order convergence.
+"""
+import numpy as np
+import pytest
+from scipy.special import ive
+
+from oracle import dmfe_oracle as O
+
+
+# ------------------------------------------------------------------------------------ P9
+def _order_conditions(A, b, c):
+    """Residuals of the 8 rooted-tree order conditions up to order 4."""
+    e = np.ones(len(b))
+    Ac = A @ c
+    return {
+        1: [b @ e - 1.0],
+        2: [b @ c - 0.5],
+        3: [b @ c ** 2 - 1 / 3, b @ Ac - 1 / 6],
+        4: [b @ c ** 3 - 0.25, b @ (c * Ac) - 1 / 8, b @ (A @ c ** 2) - 1 / 12, b @ (A @ Ac) - 1 / 24],
+    }
+
+
+def test_P9_ssprk104_order_conditions():
+    A = O.ssprk104_butcher()
+    c = A.sum(1)
+    assert np.allclose(c, O.SSPRK_C, atol=1e-15)
+    r = _order_conditions(A, O.SSPRK_B, c)
+    assert max(abs(x) for k in r for x in r[k]) < 1e-15
+    rh = _order_conditions(A, O.SSPRK_BHAT, c)
+    assert max(abs(x) for k in (1, 2, 3) for x in rh[k]) < 1e-15
+    assert max(abs(x) for x in rh[4]) > 1e-3          # embedded pair is genuinely third order
+
+
+def test_P9_low_storage_form_equals_tableau_and_converges():
+    A = O.ssprk104_butcher()
+    lam = np.array([-1.0, -0.3, 0.2])
+
+    def F(t, y):
+        return lam * y + np.sin(t)
+
+    def tableau_step(y, t0, h):
+        K = []
+        for i in range(10):
+            yi = y + h * sum(A[i, j] * K[j] for j in range(i)) if i else y
+            K.append(F(t0 + O.SSPRK_C[i] * h, yi))
+        return y + h * sum(O.SSPRK_B[i] * K[i] for i in range(10)), \
+            h * sum((O.SSPRK_B[i] - O.SSPRK_BHAT[i]) * K[i] for i in range(10))
+
+    y0 = np.array([1.0, -2.0, 0.5])
+    y1, d1 = O.ssprk104(F, y0, 0.3, 0.7)
+    y2, d2 = tableau_step(y0, 0.3, 0.7)
+    assert np.abs(y1 - y2).max() < 1e-14 and np.abs(d1 - d2).max() < 1e-14
+
+    def integrate(n):
+        y, t, h = np.array([1.0]), 0.0, 2.0 / n
+        for _ in range(n):
+            y, _d = O.ssprk104(lambda tt, yy: -yy + np.cos(tt), y, t, h)
+            t += h
+        return y[0]
+    exact = 0.5 * np.exp(-2.0) + 0.5 * (np.cos(2.0) + np.sin(2.0))
+    e1, e2 = abs(integrate(8) - exact), abs(integrate(16) - exact)
+    assert 12.0 < e1 / e2 < 20.0
+
+
+# ------------------------------------------------------------------------------------ P5
+def _Gamma(t):
+    # I1(4t)/(2t) with the exponential factored out: returns (log-free) scaled value & exponent 4t
+    return ive(1, 4 * t) / (2 * t)
+
+
+@pytest.mark.slow
+def test_P5_pure_2spin_closed_form():
+    L, s, h, nsteps = 128, 6, 0.025, 320        # t <= 8
+    grid = O.Grid(L=L, s=s, t_max=20.0)
+    model = O.Model(lam=[0.0, 0.0, 1.0], T=0.0)
+    H = O.run_fixed(grid, model, h, nsteps)
+    n = np.arange(1, H.n_rows)
+    t = H.t[n]
+    mu_ex = 2 * ive(0, 4 * t) / ive(1, 4 * t) - 1 / t
+    assert np.abs(H.mu[n] - mu_ex).max() < 5e-7
+    assert np.abs(H.E[n] + mu_ex / 2).max() < 5e-7
+    # fields on the rays of the last row and of one in the middle
+    for k in (H.n_rows - 1, H.n_rows // 2):
+        tk = H.t[k]
+        tp = grid.theta * tk
+        tau = grid.omega * tk
+        # Gamma(t) = e^{4t} _Gamma(t): C = [ive(1,2(t+t'))e^{2(t+t')}/(t+t')]/(e^{2(t+t')} sqrt(g g'))
+        tp_safe = np.maximum(tp, 1e-300)
+        g_t = _Gamma(tk)
+        g_tp = np.where(tp > 0, ive(1, 4 * tp_safe) / (2 * tp_safe), 1.0)
+        C_ex = ive(1, 2 * (tk + tp)) / (tk + tp) / np.sqrt(g_t * g_tp)
+        tau_safe = np.maximum(tau, 1e-300)
+        R_ex = np.where(tau > 0, ive(1, 2 * tau_safe) / tau_safe, 1.0) * np.sqrt(g_tp / g_t)
+        # exponentials: e^{2 tau} * e^{(4t' - 4t)/2} = 1  (they cancel exactly)
+        assert np.abs(H.hist[k, :, 0] - C_ex).max() < 2e-7
+        assert np.abs(H.hist[k, :, 2] - R_ex).max() < 1e-6
+    # 4th-order convergence in h of mu(t=2)
+    errs = []
+    for hh, ns in ((0.1, 20), (0.05, 40)):
+        Hh = O.run_fixed(grid, model, hh, ns)
+        tt = Hh.t[ns]
+        errs.append(abs(Hh.mu[ns] - (2 * ive(0, 4 * tt) / ive(1, 4 * tt) - 1 / tt)))
+    assert errs[0] / errs[1] > 6.0 or errs[1] < 5e-8
+
+
+# ------------------------------------------------------------------------------------ P6, P7
+@pytest.fixture(scope="module")
+def paramagnet_run():
+    grid = O.Grid(L=128, s=4, t_max=20.0)
+    model = O.Model(lam=[0.0, 0.0, 0.0, 1.0], T=1.0)
+    return grid, model, O.run_fixed(grid, model, 0.05, 400)
+
+
+@pytest.mark.slow
+def test_P6_constraints_hold_along_the_run(paramagnet_run):
+    grid, model, H = paramagnet_run
+    N = H.n_rows
+    assert np.abs(H.hist[:N, -1, 0] - 1.0).max() < 5e-14      # C(t,t) = 1
+    assert np.abs(H.hist[:N, -1, 2] - 1.0).max() < 5e-14      # R(t,t^-) = 1
+    assert np.abs(H.hist[:N, -1, 1]).max() < 1e-13            # ray derivative on the diagonal = 0
+    assert np.abs(H.hist[:N, -1, 3]).max() < 1e-13
+    assert np.all(H.hist[:N, :, 0] <= 1.0 + 1e-12) and np.all(H.hist[:N, :, 0] > -1e-9)
+    assert np.all(H.hist[:N, :, 2] > -1e-9)
+
+
+@pytest.mark.slow
+def test_P7_paramagnet_equilibrium_and_FDT(paramagnet_run):
+    grid, model, H = paramagnet_run
+    M = H.n_rows - 1
+    T = model.T
+    assert H.t[M] == pytest.approx(20.0, abs=1e-12)
+    assert H.mu[M] == pytest.approx(T + model.f(1.0, 1) / T, abs=2e-4)      # 2.5
+    assert H.E[M] == pytest.approx(-model.f(1.0, 0) / T, abs=1e-4)          # -0.5
+    # FDT: R(t,t') = (1/T) dC(t,t')/dt' for tau = t-t' well inside the equilibrated regime.
+    # (a) with dC/dt' from the second-argument equation evaluated by the oracle
+    out = O.history_integrals(grid, model, H.t, H.mu, H.hist, M)
+    tau = grid.omega * H.t[M]
+    sel = (tau < 8.0)
+    R = H.hist[M, :, 2]
+    assert np.abs(T * R[sel] - out["deriv"][sel, 2]).max() < 2e-3
+    # (b) with dC/dt' = (dC/di)/(t dtheta/di) by central differences in the index
+    C = H.hist[M, :, 0]
+    dCdtp = np.gradient(C) / (np.gradient(grid.theta) * H.t[M])
+    mid = sel & (tau > 0.2) & (np.arange(grid.L) < grid.L - 3)
+    assert np.abs(T * R[mid] / dCdtp[mid] - 1.0).max() < 2e-2
+    # time-translation invariance at late times: C(t, t-tau) equals C(t2, t2-tau)
+    M2 = M - 100                                   # t2 = 15
+    tau2 = grid.omega * H.t[M2]
+    Cb = np.interp(1.0, np.sort(tau2), H.hist[M2, :, 0][np.argsort(tau2)])
+    Ca = np.interp(1.0, np.sort(tau), C[np.argsort(tau)])
+    assert Ca == pytest.approx(Cb, abs=2e-3)
+
+
+# ------------------------------------------------------------------------------------ P8
+def _brute_force(lam, T, t_end, n):
+    """Uniform grid t_k = k dt; C[k][j], R[k][j] (j <= k); trapezoid memory sums; Heun in t.
+    Eq.(1) with the -mu terms of Eq.(6), Eq.(10),(11),(13), beta0 = 0."""
+    lam = np.asarray(lam, dtype=float)
+    p = np.arange(len(lam))
+
+    def f1(q):
+        return 0.5 * sum(lam[k] * k * q ** (k - 1) for k in p if k >= 1)
+
+    def f2(q):
+        return 0.5 * sum(lam[k] * k * (k - 1) * q ** (k - 2) for k in p if k >= 2)
+
+    dt = t_end / n
+    C = np.zeros((n + 1, n + 1)); R = np.zeros((n + 1, n + 1))
+    C[0, 0] = 1.0; R[0, 0] = 1.0
+    mu = np.zeros(n + 1)
+
+    def trap(y):
+        return 0.0 if len(y) < 2 else dt * (y.sum() - 0.5 * (y[0] + y[-1]))
+
+    def rhs(k, Ck, Rk):
+        """Ck, Rk = row k (entries 0..k; diagonal entries C=1, R=1).  Rows < k are in C, R."""
+        K = f2(Ck) * Rk; D = f1(Ck)
+        m = T + trap(K * Ck + D * Rk)
+        dC = np.zeros(k + 1); dR = np.zeros(k + 1)
+        for j in range(k + 1):
+            # C(s,t_j) for s = 0..k: symmetric; rows below k are stored, row k is Ck
+            Csj = np.concatenate([C[j, :j], C[j:k, j], [Ck[j]]]) if j < k else Ck.copy()
+            I1 = trap(K * Csj)
+            I2 = trap(D[:j + 1] * (R[j, :j + 1] if j < k else Rk))
+            dC[j] = -m * Ck[j] + I1 + I2
+            Rsj = np.concatenate([R[j:k, j], [Rk[j]]]) if j < k else np.array([1.0])
+            dR[j] = -m * Rk[j] + trap(K[j:] * Rsj)
+        return dC, dR, m
+
+    for k in range(n):
+        Ck, Rk = C[k, :k + 1].copy(), R[k, :k + 1].copy()
+        dC0, dR0, mu[k] = rhs(k, Ck, Rk)
+        # predictor for row k+1 (entries 0..k), diagonal appended
+        Cp = np.concatenate([Ck + dt * dC0, [1.0]]); Rp = np.concatenate([Rk + dt * dR0, [1.0]])
+        C[k + 1, :k + 2], R[k + 1, :k + 2] = Cp, Rp
+        dC1, dR1, _ = rhs(k + 1, Cp, Rp)
+        C[k + 1, :k + 1] = Ck + 0.5 * dt * (dC0 + dC1[:k + 1])
+        R[k + 1, :k + 1] = Rk + 0.5 * dt * (dR0 + dR1[:k + 1])
+        C[k + 1, k + 1] = 1.0; R[k + 1, k + 1] = 1.0
+    _, _, mu[n] = rhs(n, C[n, :n + 1].copy(), R[n, :n + 1].copy())
+    return C, R, mu
+
+
+@pytest.mark.slow
+def test_P8_uniform_grid_brute_force():
+    lam, T, t_end = [0.0, 0.0, 0.0, 1.0], 1.0, 3.0
+    Ca, Ra, mua = _brute_force(lam, T, t_end, 150)
+    Cb, Rb, mub = _brute_force(lam, T, t_end, 300)
+    # Heun + trapezoid are second order: Richardson-extrapolate the last row and mu
+    mu_x = (4 * mub[-1] - mua[-1]) / 3
+    C_x = (4 * Cb[-1, ::2] - Ca[-1]) / 3
+    R_x = (4 * Rb[-1, ::2] - Ra[-1]) / 3
+    assert abs(mub[-1] - mua[-1]) < 2e-3           # the brute force is itself converged
+    grid = O.Grid(L=192, s=4, t_max=20.0)
+    model = O.Model(lam=lam, T=T)
+    H = O.run_fixed(grid, model, 0.025, 120)
+    M = H.n_rows - 1
+    assert H.t[M] == pytest.approx(t_end, abs=1e-12)
+    assert H.mu[M] == pytest.approx(mu_x, abs=5e-5)
+    tp = np.linspace(0.0, t_end, 151)
+    # compare at the theta-grid points by interpolating the (smooth) brute-force row
+    from scipy.interpolate import CubicSpline
+    Cs = CubicSpline(tp, C_x)(grid.theta * t_end)
+    Rs = CubicSpline(tp, R_x)(grid.theta * t_end)
+    assert np.abs(H.hist[M, :, 0] - Cs).max() < 5e-5
+    assert np.abs(H.hist[M, :, 2] - Rs).max() < 5e-5
+    # and the mixed model with beta0 = 0 at lower T (different f', f'' paths)
+    lam2, T2 = [0.0, 0.0, 1.0, 0.0, 0.5], 0.5
+    C2a, R2a, mu2a = _brute_force(lam2, T2, 2.0, 100)
+    C2b, R2b, mu2b = _brute_force(lam2, T2, 2.0, 200)
+    H2 = O.run_fixed(O.Grid(L=192, s=4, t_max=20.0), O.Model(lam=lam2, T=T2), 0.025, 80)
+    assert H2.mu[H2.n_rows - 1] == pytest.approx((4 * mu2b[-1] - mu2a[-1]) / 3, abs=1e-4)
+
+
+# ------------------------------------------------------------------------------------ controller
+@pytest.mark.slow
+def test_adaptive_run_with_sparsification_is_sane():
+    """PAPER.md:320, :334 (readings G20, G25; tie-breaks are 'parity unpinned'): an adaptive
+    p=3, T=1/2 run with periodic sparsification keeps the constraints, loses rows, and heads to
+    the aging band E_inf < E(t) < E(0) with E_inf = -0.886693."""
+    grid = O.Grid(L=64, s=4, t_max=1e3)
+    model = O.Model(lam=[0.0, 0.0, 0.0, 1.0], T=0.5)
+    log = []
+    H = O.run_adaptive(grid, model, t_end=30.0, tol=1e-6, h0=1e-3, n_cap=400, sp_every=100, log=log)
+    N = H.n_rows
+    assert H.t[N - 1] >= 30.0
+    assert np.abs(H.hist[:N, -1, 0] - 1.0).max() < 1e-12
+    assert np.abs(H.hist[:N, -1, 2] - 1.0).max() < 1e-12
+    assert np.all(np.diff(H.t[:N]) > 0)
+    accepted = sum(1 for r in log if r[3])
+    assert N < accepted + 1                          # sparsification removed rows
+    assert -0.8867 < H.E[N - 1] < -0.80
+    assert all(r[2] <= 2e-6 for r in log if r[3])
