@@ -1,0 +1,157 @@
+/*
+ * dmfe.h -- C ABI of libdmfe.so: the B200 (sm_100a, fp64) hot path of the DMFE solver of
+ * arxiv/paper_2604_06309 ("DYNAMITE"): per-RK-stage evaluation of the history (memory)
+ * integrals, the device-resident SSPRK(10,4) step with its error controller, and the
+ * selective history reduction ("sparsification").
+ *
+ * Citations are PAPER.md:<line> (+ equation); readings Gnn are listed in DESIGN.md.
+ *
+ * Conventions
+ *   L        length of the fixed theta-grid, theta = t'/t in [0,1]       (Eq.(16))
+ *   rows     stored time slices t_0 = 0 < t_1 < ...; row n holds, for every theta_l,
+ *            one 32-byte cell {C, dC, R, dR}:  C(t_n, theta_l t_n), R(t_n, theta_l t_n) and their
+ *            derivatives along the ray (d/dt at fixed theta)
+ *   f(q)     = 1/2 sum_{p=0..p_max} lambda[p] q^p                        (Eq.(4); G2)
+ *   i, j, l  target node, quadrature node, stencil column (0-based)
+ *
+ * Every entry point returns 0 on success or a negative DMFE_E* code; nothing throws, nothing
+ * calls exit().  "device" pointers are CUDA device pointers owned by the caller (the Python
+ * binding takes them from torch tensors); "host" pointers are ordinary host memory.  All work is
+ * enqueued on the stream given at creation; calls that return a host scalar synchronise that
+ * stream, the others are asynchronous.  There is no CPU fallback anywhere in this library.
+ */
+#ifndef DMFE_H
+#define DMFE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define DMFE_API __attribute__((visibility("default")))
+#else
+#define DMFE_API
+#endif
+
+#define DMFE_OK 0
+#define DMFE_EINVAL (-1)      /* bad parameter (L < 2s, t_max <= e, n_rows < 2, NULL pointer ...) */
+#define DMFE_ECUDA (-2)       /* a CUDA call failed; dmfe_last_cuda_error() has the code          */
+#define DMFE_ECAPACITY (-3)   /* append with n_rows == n_cap, or a forced sparsify freed nothing  */
+#define DMFE_ESTEPMIN (-4)    /* controller drove h below h_min                    */
+#define DMFE_ENONFINITE (-5)  /* eps_RK not finite and nothing left to revert                     */
+#define DMFE_ENOMEM (-6)      /* host or device allocation failed                                 */
+
+typedef struct dmfe_ctx dmfe_ctx; /* opaque: tables + O(L) scratch on the device */
+
+typedef struct {
+  int32_t L;           /* theta-grid length, >= 2*stencil                                        */
+  int32_t stencil;     /* s = points of the index-Lagrange stencil, even, 2..10   */
+  int32_t quad_degree; /* odd degree of the global spline that defines nu_j; 5 = paper default
+                          (PAPER.md:278); 1 and 3 are accepted                                   */
+  int32_t p_max;       /* lambda has p_max+1 entries, 2 <= p_max <= 15                           */
+  double t_max;        /* sets gamma = -W_{-1}(-1/t_max); must be > e             */
+  double beta0;        /* inverse temperature of the initial condition, 0 = random start (Eq.(12)) */
+  double tol;          /* epsilon of Eq.(25); used by rk_step / sparsify only      */
+  double h_min;        /* terminate below this step; 0 -> 1e-12                    */
+  void *stream;        /* cudaStream_t borrowed from the caller (0 = default stream)             */
+} dmfe_params;
+
+/* Build the t-independent tables ("precomputed once"): theta_i and the complement
+ * omega_i = 1-theta_i (Eq.(16)), quadrature weights nu_j, and for every pair
+ * (i,j) and each coordinate phi1 = theta_i theta_j, phi2 = theta_i + omega_i theta_j,
+ * psi = theta_i/phi2 the stencil start and the fractional index coordinate
+ * (Eq.(18), (20)).  lambda: host, [p_max+1].  T: bath temperature.  *out receives the context. */
+DMFE_API int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_ctx **out);
+DMFE_API int dmfe_destroy(dmfe_ctx *ctx);
+
+/* Last CUDA error code seen by this context (cudaError_t as int), 0 if none. */
+DMFE_API int dmfe_last_cuda_error(const dmfe_ctx *ctx);
+DMFE_API const char *dmfe_strerror(int code);
+
+/* Test hook (table parity): copy tables to HOST buffers.  theta, omega, nu: [L] (any may be NULL).
+ * start: [3][n_targets][L] int32, frac: [3][n_targets][L] fp64 for the coordinates
+ * (phi1, phi2, psi) of targets i0 .. i0+n_targets-1 (NULL to skip).  Synchronises. */
+DMFE_API int dmfe_get_tables(dmfe_ctx *ctx, double *theta, double *omega, double *nu, int32_t i0,
+                    int32_t n_targets, int32_t *start, double *frac);
+
+/* The history as the caller holds it (all DEVICE pointers, caller-owned). */
+typedef struct {
+  int32_t n_rows;     /* rows 0..n_rows-1 are valid; row M = n_rows-1 is the CURRENT row: its
+                         derivative slots and mu[M] are ignored on input (G12)                  */
+  int32_t n_cap;      /* row capacity of the three arrays                                       */
+  const double *t;    /* [n_cap] ascending, t[0] = 0                                            */
+  const double *mu;   /* [n_cap] Lagrange multiplier of rows 0..M-1 (Eq.(13))                   */
+  const double *hist; /* [n_cap][L][4] packed cells {C, dC, R, dR}                              */
+} dmfe_grid;
+
+/* Outputs of one right-hand-side evaluation; DEVICE pointers, any may be NULL. */
+typedef struct {
+  double *d1C;    /* [L] dC/dt  of Eq.(1) (with the -mu C term, G1)              */
+  double *d1R;    /* [L] dR/dt  of Eq.(1)                                                        */
+  double *mu;     /* [1] mu(t), Eq.(13)                                           */
+  double *d2C;    /* [L] dC/dt' (second-argument equation, G9/G10)                               */
+  double *d2R;    /* [L] dR/dt'                                                                  */
+  double *F;      /* [L][2] ray derivatives {d1C + theta d2C, d1R + theta d2R} = ODE rhs, Eq.(22) */
+  double *energy; /* [1] E(t), Eq.(14)                                            */
+  double *sums;   /* [8][L] the eight nu-weighted sums S1..S8 of Eq.(21) (DESIGN.md step 6)      */
+  int32_t *rows1; /* [L]    test hook: type-1 row index n(theta_i t)                             */
+  int32_t *rows2; /* [L][L] test hook: type-2 row index n(phi2_ij t)                             */
+} dmfe_rhs_out;
+
+/* north-star call (grid, C, R, t_n) -> (dC, dR, mu): C, R are row M of grid->hist, t_n = t[M].
+ * Eq.(17)-(21) with K = f''(C)R, D = f'(C) (Eq.(10)-(11)).  Asynchronous. */
+DMFE_API int dmfe_history_integrals(dmfe_ctx *ctx, const dmfe_grid *grid, const dmfe_rhs_out *out);
+
+/* Same call with HOST buffers (the end-to-end leg of bench.py): copies t, mu, hist rows
+ * 0..n_rows-1 to library-owned device staging (grown on demand), evaluates, copies
+ * d1C, d1R [L] and mu, energy [1] back (any may be NULL).  Synchronises. */
+DMFE_API int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const double *t, const double *mu_hist,
+                                const double *hist, double *d1C, double *d1R, double *mu,
+                                double *energy);
+
+/* Device-resident integrator state.  The arrays are caller-owned DEVICE memory. */
+typedef struct {
+  int32_t n_rows;  /* complete rows (value + derivative + mu); updated by the library            */
+  int32_t n_cap;   /* capacity; a step needs n_rows + 1 <= n_cap - 1                              */
+  double *t;       /* [n_cap]                                                                     */
+  double *mu;      /* [n_cap]                                                                     */
+  double *energy;  /* [n_cap] E(t_n) of every stored row                                          */
+  double *hist;    /* [n_cap][L][4]                                                               */
+  double h;        /* current step size (host copy; the device copy lives in the context)        */
+  double eps_rk;   /* Eq.(25) of the last attempted step (host copy)                              */
+  int64_t n_rhs;   /* history-integral evaluations so far                                         */
+} dmfe_state;
+
+/* Row 0 at t = 0 (G13): C = R = 1, ray slopes -T(1-theta), -mu0(1-theta), mu0 = T + beta0 f'(1);
+ * sets n_rows = 1 and h = h0 (capped by the stability bound of Eq.(24)). */
+DMFE_API int dmfe_init_state(dmfe_ctx *ctx, dmfe_state *st, double h0);
+
+/* One SSPRK(10,4) step from the last row, all stages on the device.
+ * fixed_step != 0: no controller, the row is always appended.  Otherwise the controller of
+ * PAPER.md:320 (G20): eps_RK > 2 tol or non-finite -> drop the last 10 rows, h/2, *accepted = 0;
+ * else append, h *= 0.9 if eps_RK > tol, h *= 1.01 if eps_RK < tol/2, *accepted = 1.
+ * Exactly one scalar record returns to the host per call. */
+DMFE_API int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *accepted);
+
+/* Selective history reduction, Eq.(26)-(27): drop row n if eps_sparse < tol/10,
+ * then skip to n+2; row 0 and the last protect_last rows are kept; t, mu, energy and the packed
+ * rows are compacted on the device.  keep_mask: optional HOST [n_rows before] bytes (test hook). */
+DMFE_API int dmfe_sparsify(dmfe_ctx *ctx, dmfe_state *st, int32_t protect_last, int32_t *n_rows_out,
+                  uint8_t *keep_mask);
+
+/* Measurement hooks (bench.py).  dmfe_enable_timing: when on, every dmfe_history_integrals launch
+ * records CUDA events on the context's stream immediately before and after the pair kernel (the
+ * dominant kernel); dmfe_last_kernel_ms synchronises on the closing event and returns the elapsed
+ * time of the most recent one.  dmfe_probe_fp64_tflops runs a register-resident DFMA chain on all
+ * SMs (n_iter fused multiply-adds per thread, 8 independent chains) and reports the achieved
+ * 2*DFMA/s: the denominator of the FP64 roofline, measured rather than assumed. */
+DMFE_API int dmfe_enable_timing(dmfe_ctx *ctx, int32_t on);
+DMFE_API int dmfe_last_kernel_ms(dmfe_ctx *ctx, float *ms);
+DMFE_API int dmfe_probe_fp64_tflops(dmfe_ctx *ctx, int32_t n_iter, double *tflops, int32_t *sm_count);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DMFE_H */

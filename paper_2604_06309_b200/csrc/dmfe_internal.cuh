@@ -1,0 +1,87 @@
+// Internal declarations of libdmfe.so (not part of the C ABI; see include/dmfe.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dmfe.h"
+
+#define DMFE_PMAX_MAX 15
+
+// f(q) = 1/2 sum_p lambda_p q^p (Eq.(4)).  Horner coefficients, lowest power first:
+//   f (q) = sum_k c0[k] q^k        c0[k] = lambda_k / 2
+//   f'(q) = sum_k c1[k] q^k        c1[k] = (k+1) lambda_{k+1} / 2
+//   f''(q)= sum_k c2[k] q^k        c2[k] = (k+2)(k+1) lambda_{k+2} / 2
+struct ModelCoef {
+  double c0[DMFE_PMAX_MAX + 1];
+  double c1[DMFE_PMAX_MAX + 1];
+  double c2[DMFE_PMAX_MAX + 1];
+  double T;
+  double beta0;
+  int32_t pmax;
+};
+
+// device scalar block (ctx->scal), indices
+enum {
+  SC_MU = 0,     // mu(t) of the row being evaluated (Eq.(13))
+  SC_E = 1,      // E(t) (Eq.(14))
+  SC_H = 2,      // current step size
+  SC_EPS = 3,    // eps_RK of the last attempted step (Eq.(25))
+  SC_T0 = 4,     // t_N at the start of the step
+  SC_HNEXT = 5,  // step size proposed by the controller
+  SC_COUNT = 16
+};
+// device int block (ctx->iscal)
+enum {
+  IS_ACCEPT = 0,  // 1 accepted, 0 reverted
+  IS_NROWS = 1,   // complete rows after the step / after sparsify
+  IS_FIRST = 2,   // sparsify: first row that moves
+  IS_COUNT = 8
+};
+
+struct dmfe_ctx {
+  dmfe_params p;
+  ModelCoef model;
+  cudaStream_t stream;
+  int cuda_err;
+  double gamma, A, B;  // gamma = -W_{-1}(-1/t_max); A = atan(e^gamma), B = atan(e^-gamma)
+  double h_stab;       // 13.9 / (4 sqrt(f''(1)))  (Eq.(24))
+  // ---- tables (device) ----
+  double *theta, *omega, *nu;  // [L]
+  int32_t *start;              // [3][L][L]
+  double *frac;                // [3][L][L]
+  // ---- O(L) scratch (device) ----
+  double2 *cur;     // [L] {C, R} of the current row, packed for 16-byte gathers
+  double *scal;     // [SC_COUNT]
+  int32_t *iscal;   // [IS_COUNT]
+  double *rk;       // [4][L][2]: q1, q2, delta, F
+  double *eps_sp;   // [n] sparsify residuals (grown on demand)
+  int32_t *keep;    // [n] keep flags / scan
+  int32_t *newidx;  // [n] compacted source index
+  int32_t sp_cap;
+  double *row_tmp;  // staging for compaction
+  size_t row_tmp_bytes;
+  // ---- host-buffer leg ----
+  double *stage_t, *stage_mu, *stage_hist, *stage_out;
+  int32_t stage_rows;
+  // measurement hooks
+  int timing_on;
+  cudaEvent_t ev0, ev1;
+  // pinned host scalars for the one-record-per-step readback
+  double *h_scal;
+  int32_t *h_iscal;
+};
+
+#define CUDA_TRY(ctx, call)                              \
+  do {                                                   \
+    cudaError_t e__ = (call);                            \
+    if (e__ != cudaSuccess) {                            \
+      (ctx)->cuda_err = (int)e__;                        \
+      return DMFE_ECUDA;                                 \
+    }                                                    \
+  } while (0)
+
+// tables.cu
+int dmfe_build_tables(dmfe_ctx *ctx);
+// history_integrals.cu
+int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, const double *t, const double *mu_hist, const double *hist,
+                    const dmfe_rhs_out *out);

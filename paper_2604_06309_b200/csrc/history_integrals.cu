@@ -1,0 +1,328 @@
+// The per-RK-stage history integrals (section 3.3-3.4): for every target theta_i and
+// quadrature node theta_j
+//   A factors    C1,R1 = row M at phi1_ij, C2,R2 = row M at phi2_ij     (Eq.(18))
+//   type-1       B1C,B1R = history at (theta_i t, theta_j): Hermite in t  (Eq.(19))
+//   type-2       B2C,B2R = history at (phi2_ij t, psi_ij): theta-stencil, then Hermite in t after a
+//                row search                                             (Eq.(20))
+//   kernels      K = f''(C) R, D = f'(C)                                 (Eq.(10)-(11))
+//   sums         eight nu-weighted sums over j                           (Eq.(21))
+// and the O(L) parts: mu(t) Eq.(13), E(t) Eq.(14), the right-hand sides of Eq.(1) and of the
+// second-argument equations (readings G1, G9, G10 in DESIGN.md), the ray derivative of Eq.(22).
+//
+// Mapping: one CTA per target i, lanes <-> adjacent nodes j (type-1 rows and the pair tables are
+// read coalesced; the type-2 cells of adjacent lanes are neighbours in the packed history).
+// Every history cell {C,dC,R,dR} is one 256-bit load.  fp64 throughout; no tensor cores: every
+// "matrix" here is a gather.
+#include "dmfe_internal.cuh"
+
+namespace {
+
+constexpr int RHS_THREADS = 256;
+
+struct RhsArgs {
+  int32_t L, M;
+  const double *theta, *omega, *nu;
+  const int32_t *start;
+  const double *frac;
+  const double *t, *mu_hist;
+  const double4 *hist;
+  const double2 *cur;
+  const double *scal;  // SC_MU, SC_E written by pack_mu_energy_kernel
+  dmfe_rhs_out out;
+};
+
+__device__ __forceinline__ double4 ld_cell(const double4 *p) {
+  double4 v;
+  asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+               : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w)
+               : "l"(p));
+  return v;
+}
+
+__device__ __forceinline__ double horner(const double *c, int deg, double q) {
+  double acc = c[deg];
+  for (int k = deg - 1; k >= 0; --k) acc = fma(acc, q, c[k]);
+  return acc;
+}
+
+// Lagrange cardinal weights on the integer nodes 0..S-1 at u (PAPER.md:236 index interpolation):
+// w_l = prod_{m<l}(u-m) * prod_{m>l}(u-m) / prod_{m!=l}(l-m)
+template <int S>
+__device__ __forceinline__ void lagrange_weights(double u, double (&w)[S]) {
+  double d[S], pre[S], suf[S];
+#pragma unroll
+  for (int m = 0; m < S; ++m) d[m] = u - (double)m;
+  pre[0] = 1.0;
+#pragma unroll
+  for (int m = 1; m < S; ++m) pre[m] = pre[m - 1] * d[m - 1];
+  suf[S - 1] = 1.0;
+#pragma unroll
+  for (int m = S - 2; m >= 0; --m) suf[m] = suf[m + 1] * d[m + 1];
+#pragma unroll
+  for (int l = 0; l < S; ++l) {
+    double den = 1.0;
+#pragma unroll
+    for (int m = 0; m < S; ++m)
+      if (m != l) den *= (double)(l - m);
+    w[l] = pre[l] * suf[l] * (1.0 / den);  // 1/den folds to a compile-time constant
+  }
+}
+
+// n = max{ n <= M-1 : t[n] <= tau }; t ascending, t[0] = 0 <= tau.
+__device__ __forceinline__ int row_search(const double *__restrict__ t, int M, double tau) {
+  int lo = 0, hi = M - 1;
+  while (lo < hi) {
+    const int mid = lo + ((hi - lo + 1) >> 1);
+    if (__ldg(t + mid) <= tau)
+      lo = mid;
+    else
+      hi = mid - 1;
+  }
+  return lo;
+}
+
+// weights of the local interpolant in t between rows n and n+1 (PAPER.md:260 cubic Hermite);
+// quadratic (value, slope, value) when the upper row is the current row M (reading G12).
+__device__ __forceinline__ void t_weights(double tn, double tn1, double tau, bool top, double (&h)[4]) {
+  const double D = tn1 - tn;
+  const double u = (tau - tn) / D;
+  const double u2 = u * u;
+  if (top) {
+    h[0] = 1.0 - u2;
+    h[1] = (u - u2) * D;
+    h[2] = u2;
+    h[3] = 0.0;
+  } else {
+    const double u3 = u2 * u;
+    h[0] = 2.0 * u3 - 3.0 * u2 + 1.0;
+    h[1] = (u3 - 2.0 * u2 + u) * D;
+    h[2] = 3.0 * u2 - 2.0 * u3;
+    h[3] = (u3 - u2) * D;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// O(L) pre-pass: pack row M into {C,R} pairs and reduce mu(t) (Eq.(13)) and E(t) (Eq.(14)).
+__global__ void __launch_bounds__(1024) pack_mu_energy_kernel(int L, int M, ModelCoef mc,
+                                                              const double *__restrict__ nu,
+                                                              const double *__restrict__ t,
+                                                              const double4 *__restrict__ hist,
+                                                              double2 *__restrict__ cur,
+                                                              double *__restrict__ scal) {
+  __shared__ double sm[32], se[32];
+  const double4 *row = hist + (size_t)M * (size_t)L;
+  double am = 0.0, ae = 0.0;
+  for (int j = threadIdx.x; j < L; j += blockDim.x) {
+    const double4 c = ld_cell(row + j);
+    cur[j] = make_double2(c.x, c.z);
+    const double fp = horner(mc.c1, mc.pmax - 1, c.x), fpp = horner(mc.c2, mc.pmax - 2, c.x);
+    const double nj = nu[j];
+    am += nj * (fpp * c.z * c.x + fp * c.z);
+    ae += nj * (fp * c.z);
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    am += __shfl_xor_sync(0xffffffffu, am, o);
+    ae += __shfl_xor_sync(0xffffffffu, ae, o);
+  }
+  const int w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  if ((threadIdx.x & 31) == 0) sm[w] = am, se[w] = ae;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double tm = 0.0, te = 0.0;
+    for (int k = 0; k < nw; ++k) tm += sm[k], te += se[k];
+    const double tM = t[M];
+    const double c0 = row[0].x;
+    scal[SC_MU] = mc.T + tM * tm + mc.beta0 * horner(mc.c1, mc.pmax - 1, c0) * c0;
+    scal[SC_E] = -tM * te - mc.beta0 * horner(mc.c0, mc.pmax, c0);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+template <int S>
+__global__ void __launch_bounds__(RHS_THREADS) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
+  const int L = a.L, M = a.M;
+  const int i = blockIdx.x;
+  const size_t plane = (size_t)L * (size_t)L;
+  const size_t rowoff = (size_t)i * (size_t)L;
+  const double th_i = a.theta[i], om_i = a.omega[i];
+  const double tM = a.t[M];
+  const int d1 = mc.pmax - 1, d2 = mc.pmax - 2;
+
+  // type-1: one row search per target, tau = theta_i t  (Eq.(19))
+  const double tau1 = __dmul_rn(th_i, tM);
+  const int n1 = row_search(a.t, M, tau1);
+  const bool top1 = (n1 + 1 == M);
+  double h1[4];
+  t_weights(a.t[n1], a.t[n1 + 1], tau1, top1, h1);
+  const double4 *row1lo = a.hist + (size_t)n1 * (size_t)L;
+  const double4 *row1hi = row1lo + L;
+
+  double acc[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) acc[k] = 0.0;
+  __shared__ double red[RHS_THREADS / 32][8];
+  __shared__ double b1c_first;
+
+  for (int j = threadIdx.x; j < L; j += RHS_THREADS) {
+    const size_t e = rowoff + (size_t)j;
+    const int a1 = __ldg(a.start + e), a2 = __ldg(a.start + plane + e), a3 = __ldg(a.start + 2 * plane + e);
+    const double u1 = __ldg(a.frac + e), u2 = __ldg(a.frac + plane + e), u3 = __ldg(a.frac + 2 * plane + e);
+    double w[S];
+    // ---- A factors on the current row (Eq.(18)) ----
+    double C1 = 0.0, R1 = 0.0, C2 = 0.0, R2 = 0.0;
+    lagrange_weights<S>(u1, w);
+#pragma unroll
+    for (int l = 0; l < S; ++l) {
+      const double2 v = __ldg(a.cur + a1 + l);
+      C1 = fma(w[l], v.x, C1);
+      R1 = fma(w[l], v.y, R1);
+    }
+    lagrange_weights<S>(u2, w);
+#pragma unroll
+    for (int l = 0; l < S; ++l) {
+      const double2 v = __ldg(a.cur + a2 + l);
+      C2 = fma(w[l], v.x, C2);
+      R2 = fma(w[l], v.y, R2);
+    }
+    // ---- type-1 lookup (Eq.(19)) ----
+    const double4 lo = ld_cell(row1lo + j);
+    double4 hi = ld_cell(row1hi + j);
+    if (top1) hi.y = 0.0, hi.w = 0.0;
+    const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
+    const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
+    if (j == 0) b1c_first = B1C;
+    // ---- type-2 lookup (Eq.(20)): theta-stencil first, then t ----
+    const double th_j = a.theta[j];
+    const double phi2 = __dadd_rn(th_i, __dmul_rn(om_i, th_j));
+    const double tau2 = __dmul_rn(phi2, tM);
+    const int n2 = row_search(a.t, M, tau2);
+    if (a.out.rows2) a.out.rows2[e] = n2;
+    const bool top2 = (n2 + 1 == M);
+    double h2[4];
+    t_weights(__ldg(a.t + n2), __ldg(a.t + n2 + 1), tau2, top2, h2);
+    lagrange_weights<S>(u3, w);
+    const double4 *p2 = a.hist + (size_t)n2 * (size_t)L + a3;
+    double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
+#pragma unroll
+    for (int l = 0; l < S; ++l) {
+      const double4 x = ld_cell(p2 + l);
+      const double4 y = ld_cell(p2 + L + l);
+      cl = fma(w[l], x.x, cl);
+      dcl = fma(w[l], x.y, dcl);
+      rl = fma(w[l], x.z, rl);
+      drl = fma(w[l], x.w, drl);
+      cu = fma(w[l], y.x, cu);
+      dcu = fma(w[l], y.y, dcu);
+      ru = fma(w[l], y.z, ru);
+      dru = fma(w[l], y.w, dru);
+    }
+    if (top2) dcu = 0.0, dru = 0.0;
+    const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
+    const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
+    // ---- kernel functions (Eq.(10)-(11)) and the eight terms (Eq.(21)) ----
+    const double nj = a.nu[j];
+    const double K1 = nj * (horner(mc.c2, d2, C1) * R1);
+    const double K2 = nj * (horner(mc.c2, d2, C2) * R2);
+    acc[0] = fma(K1, B1C, acc[0]);                                   // S1: K(t,s) C(t',s)
+    acc[1] = fma(K2, B2C, acc[1]);                                   // S2: K(t,s) C(s,t')
+    acc[2] = fma(nj * horner(mc.c1, d1, C1), B1R, acc[2]);           // S3: D(t,s) R(t',s)
+    acc[3] = fma(K2, B2R, acc[3]);                                   // S4: K(t,s) R(s,t')
+    acc[4] = fma(nj * (horner(mc.c2, d2, B1C) * B1R), C1, acc[4]);   // S5: K(t',s) C(t,s)
+    acc[5] = fma(nj * horner(mc.c1, d1, B1C), R1, acc[5]);           // S6: D(t',s) R(t,s)
+    acc[6] = fma(nj * horner(mc.c1, d1, B2C), R2, acc[6]);           // S7: D(s,t') R(t,s)
+    acc[7] = fma(nj * R2, horner(mc.c2, d2, B2C) * B2R, acc[7]);     // S8: R(t,s) K(s,t')
+  }
+
+  // ---- reduction over j: shuffle within the warp, fixed order across warps ----
+#pragma unroll
+  for (int k = 0; k < 8; ++k)
+    for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
+  const int wid = threadIdx.x >> 5;
+  if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) red[wid][k] = acc[k];
+  }
+  __syncthreads();
+  if (threadIdx.x != 0) return;
+
+  double Sd[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    double s = 0.0;
+    for (int w = 0; w < RHS_THREADS / 32; ++w) s += red[w][k];
+    Sd[k] = s;
+    if (a.out.sums) a.out.sums[(size_t)k * L + i] = s;
+  }
+  if (a.out.rows1) a.out.rows1[i] = n1;
+
+  // ---- combine (Eq.(1), second-argument equations, Eq.(22)) ----
+  const double mu = a.scal[SC_MU];
+  // mu(theta_i t): local 4-point Lagrange in t over rows k..k+3 (reading G11), mu_M = mu
+  const int npts = (M + 1 < 4) ? M + 1 : 4;
+  int k0 = n1 - 1;
+  if (k0 > M + 1 - npts) k0 = M + 1 - npts;
+  if (k0 < 0) k0 = 0;
+  double mu_p = 0.0;
+  for (int p = 0; p < npts; ++p) {
+    double wgt = 1.0;
+    for (int q = 0; q < npts; ++q)
+      if (q != p) wgt *= (tau1 - a.t[k0 + q]) / (a.t[k0 + p] - a.t[k0 + q]);
+    const double mv = (k0 + p == M) ? mu : a.mu_hist[k0 + p];
+    mu_p += wgt * mv;
+  }
+  const double2 ci = a.cur[i], c0 = a.cur[0];
+  const double fc = mc.beta0 * horner(mc.c1, d1, c0.x) * b1c_first;
+  const double fc2 = mc.beta0 * horner(mc.c1, d1, b1c_first) * c0.x;
+  const double d1C = -mu * ci.x + tM * (th_i * Sd[0] + om_i * Sd[1] + th_i * Sd[2]) + fc;
+  const double d1R = -mu * ci.y + tM * (om_i * Sd[3]);
+  const double d2C = -mu_p * ci.x + tM * (th_i * Sd[4] + th_i * Sd[5] + om_i * Sd[6]) + 2.0 * mc.T * ci.y + fc2;
+  const double d2R = mu_p * ci.y - tM * (om_i * Sd[7]);
+  if (a.out.d1C) a.out.d1C[i] = d1C;
+  if (a.out.d1R) a.out.d1R[i] = d1R;
+  if (a.out.d2C) a.out.d2C[i] = d2C;
+  if (a.out.d2R) a.out.d2R[i] = d2R;
+  if (a.out.F) {
+    a.out.F[2 * i] = d1C + th_i * d2C;
+    a.out.F[2 * i + 1] = d1R + th_i * d2R;
+  }
+  if (i == 0) {
+    if (a.out.mu) a.out.mu[0] = mu;
+    if (a.out.energy) a.out.energy[0] = a.scal[SC_E];
+  }
+}
+
+}  // namespace
+
+// M = index of the current row; its time t[M] is read on the device (the RK step keeps t there).
+int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, const double *t, const double *mu_hist, const double *hist,
+                    const dmfe_rhs_out *out) {
+  const int L = ctx->p.L;
+  pack_mu_energy_kernel<<<1, 1024, 0, ctx->stream>>>(L, M, ctx->model, ctx->nu, t, (const double4 *)hist,
+                                                     ctx->cur, ctx->scal);
+  RhsArgs a;
+  a.L = L;
+  a.M = M;
+  a.theta = ctx->theta;
+  a.omega = ctx->omega;
+  a.nu = ctx->nu;
+  a.start = ctx->start;
+  a.frac = ctx->frac;
+  a.t = t;
+  a.mu_hist = mu_hist;
+  a.hist = (const double4 *)hist;
+  a.cur = ctx->cur;
+  a.scal = ctx->scal;
+  a.out = *out;
+  if (ctx->timing_on) CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+  switch (ctx->p.stencil) {
+    case 2: history_integrals_kernel<2><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
+    case 4: history_integrals_kernel<4><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
+    case 6: history_integrals_kernel<6><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
+    case 8: history_integrals_kernel<8><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
+    case 10: history_integrals_kernel<10><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
+    default: return DMFE_EINVAL;
+  }
+  if (ctx->timing_on) CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+  CUDA_TRY(ctx, cudaGetLastError());
+  return DMFE_OK;
+}

@@ -1,0 +1,77 @@
+// Measurement hooks of include/dmfe.h: per-launch timing of the pair kernel and a DFMA-only
+// throughput probe (the FP64 roofline denominator is measured on the box, not assumed).
+#include "dmfe_internal.cuh"
+
+namespace {
+
+__global__ void __launch_bounds__(256) dfma_chain_kernel(int n_iter, double a, double b, double *sink) {
+  double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+  for (int k = 0; k < n_iter; k += 8) {
+#pragma unroll
+    for (int u = 0; u < 1; ++u) {
+      x0 = fma(x0, a, b);
+      x1 = fma(x1, a, b);
+      x2 = fma(x2, a, b);
+      x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b);
+      x5 = fma(x5, a, b);
+      x6 = fma(x6, a, b);
+      x7 = fma(x7, a, b);
+    }
+  }
+  const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (s == 123.456) sink[0] = s;  // never true; keeps the chain alive
+}
+
+}  // namespace
+
+extern "C" {
+
+int dmfe_enable_timing(dmfe_ctx *ctx, int32_t on) {
+  if (!ctx) return DMFE_EINVAL;
+  ctx->timing_on = on ? 1 : 0;
+  return DMFE_OK;
+}
+
+int dmfe_last_kernel_ms(dmfe_ctx *ctx, float *ms) {
+  if (!ctx || !ms || !ctx->timing_on) return DMFE_EINVAL;
+  CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev1));
+  CUDA_TRY(ctx, cudaEventElapsedTime(ms, ctx->ev0, ctx->ev1));
+  return DMFE_OK;
+}
+
+int dmfe_probe_fp64_tflops(dmfe_ctx *ctx, int32_t n_iter, double *tflops, int32_t *sm_count) {
+  if (!ctx || !tflops || n_iter < 8) return DMFE_EINVAL;
+  int dev = 0, sms = 0;
+  CUDA_TRY(ctx, cudaGetDevice(&dev));
+  CUDA_TRY(ctx, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  if (sm_count) *sm_count = sms;
+  n_iter -= n_iter % 8;
+  const int blocks = sms * 8, threads = 256;
+  cudaEvent_t e0, e1;
+  CUDA_TRY(ctx, cudaEventCreate(&e0));
+  CUDA_TRY(ctx, cudaEventCreate(&e1));
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0, ctx->stream);
+    dfma_chain_kernel<<<blocks, threads, 0, ctx->stream>>>(n_iter, 0.999999, 1e-7, ctx->scal + SC_COUNT - 1);
+    cudaEventRecord(e1, ctx->stream);
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e != cudaSuccess) {
+      cudaEventDestroy(e0);
+      cudaEventDestroy(e1);
+      ctx->cuda_err = (int)e;
+      return DMFE_ECUDA;
+    }
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  const double flops = 2.0 * (double)n_iter * (double)blocks * (double)threads;
+  *tflops = flops / ((double)best * 1e-3) / 1e12;
+  return DMFE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,210 @@
+"""GPU parity: libdmfe.so (through its C ABI, via the ctypes binding) against the CPU oracle on
+identical seeded inputs.  Stage A tables, Stage B single right-hand side, edge cases.
+
+Tolerances: integer results (stencil starts, row indices) bit-exact; each of
+the eight sums within 1e-12 * sum_j |term| (north_star: 1e-12 relative, different summation
+order); mu, E 1e-12 relative; combined derivatives within 1e-12 of their magnitude scale.
+"""
+import numpy as np
+import pytest
+
+from oracle import dmfe_oracle as O
+from paper_2604_06309_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def D():
+    from paper_2604_06309_b200 import dmfe
+    dmfe.load_library()  # fails loudly if the CUDA library is missing
+    return dmfe
+
+
+def _oracle_grid_from_library(tab, L, s, t_max):
+    return O.Grid(L=L, s=s, t_max=t_max, theta=tab["theta"], omega=tab["omega"], nu=tab["nu"])
+
+
+def gpu_rhs(D, ctx, L, t, mu, hist, n_rows, want_rows=True):
+    import torch
+    dev = "cuda"
+    tt = torch.from_numpy(np.ascontiguousarray(t)).to(dev)
+    tm = torch.from_numpy(np.ascontiguousarray(mu)).to(dev)
+    th = torch.from_numpy(np.ascontiguousarray(hist)).to(dev)
+    z = lambda *shape: torch.full(shape, float("nan"), dtype=torch.float64, device=dev)
+    out = dict(d1C=z(L), d1R=z(L), mu_out=z(1), d2C=z(L), d2R=z(L), F=z(L, 2), energy=z(1), sums=z(8, L))
+    if want_rows:
+        out["rows1"] = torch.full((L,), -1, dtype=torch.int32, device=dev)
+        out["rows2"] = torch.full((L, L), -1, dtype=torch.int32, device=dev)
+    D.dmfe_history_integrals(ctx, n_rows, tt, tm, th, **out)
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in out.items()}
+
+
+def compare_rhs(g, ref, tol=RTOL):
+    """g: GPU outputs, ref: oracle outputs (dict of history_integrals)."""
+    if "rows1" in g:
+        assert np.array_equal(g["rows1"], ref["rows1"]), "type-1 row indices differ"
+        assert np.array_equal(g["rows2"], ref["rows2"]), "type-2 row indices differ"
+    sums = g["sums"].T  # [L,8]
+    err = np.abs(sums - ref["sums"])
+    bound = tol * ref["abssums"] + 1e-300
+    worst = np.max(err / bound)
+    assert worst <= 1.0, "sums off by %.3g x tolerance" % worst
+    assert abs(g["mu_out"][0] - ref["mu"]) <= tol * abs(ref["mu"])
+    assert abs(g["energy"][0] - ref["E"]) <= tol * max(abs(ref["E"]), 1e-300)
+    d = ref["deriv"]
+    sc = ref["scale"]
+    for k, name in enumerate(["d1C", "d1R", "d2C", "d2R"]):
+        e = np.abs(g[name] - d[:, k])
+        w = np.max(e / (tol * sc[:, k] + 1e-300))
+        assert w <= 1.0, "%s off by %.3g x tolerance" % (name, w)
+    th = ref["theta"]
+    scF = np.stack([sc[:, 0] + th * sc[:, 2], sc[:, 1] + th * sc[:, 3]], axis=1)
+    e = np.abs(g["F"] - d[:, 4:6])
+    assert np.max(e / (tol * scF + 1e-300)) <= 1.0
+
+
+# ------------------------------------------------------------------------------------ Stage A
+@pytest.mark.parametrize("L,s,t_max", [(128, 4, 20.0), (257, 6, 1e7), (512, 4, 1e4), (96, 10, 1e5)])
+def test_tables_match_oracle(D, L, s, t_max):
+    ctx = D.dmfe_create(L, s, t_max, [0, 0, 0, 1.0], T=1.0)
+    try:
+        tab = D.dmfe_get_tables(ctx, L)
+    finally:
+        D.dmfe_destroy(ctx)
+    ref = O.Grid(L=L, s=s, t_max=t_max)
+    # grid: endpoints exact, symmetric complement, relative 1e-13 against the oracle's own grid
+    assert tab["theta"][0] == 0.0 and tab["theta"][-1] == 1.0
+    assert np.array_equal(tab["omega"], tab["theta"][::-1])
+    assert np.all(np.diff(tab["theta"]) > 0)
+    np.testing.assert_allclose(tab["theta"][1:], ref.theta[1:], rtol=1e-13, atol=0)
+    # quadrature weights: relative 1e-10 (spline solve) and the pin P2 on the library's own weights
+    np.testing.assert_allclose(tab["nu"], ref.nu, rtol=1e-10, atol=1e-10 * np.max(np.abs(ref.nu)))
+    for k in range(6):
+        assert abs(np.sum(tab["nu"] * tab["theta"] ** k) - 1.0 / (k + 1)) < 5e-14
+    # pair tables: the oracle recomputes them from the library's theta/omega
+    g2 = _oracle_grid_from_library(tab, L, s, t_max)
+    start, frac = g2.tables()
+    assert np.array_equal(tab["start"], start), "stencil starts are not bit-exact"
+    assert np.max(np.abs(tab["frac"] - frac)) <= 1e-11
+
+
+def test_tables_row_range_hook(D):
+    L, s = 128, 4
+    ctx = D.dmfe_create(L, s, 1e4, [0, 0, 1.0, 0, 0.5], T=0.5)
+    try:
+        full = D.dmfe_get_tables(ctx, L)
+        part = D.dmfe_get_tables(ctx, L, i0=17, n_targets=9)
+    finally:
+        D.dmfe_destroy(ctx)
+    assert np.array_equal(part["start"], full["start"][:, 17:26])
+    assert np.array_equal(part["frac"], full["frac"][:, 17:26])
+
+
+# ------------------------------------------------------------------------------------ Stage B
+CASES = [
+    # L, N, s, lam, T, beta0, t_max, t_end
+    (96, 37, 4, [0, 0, 0, 1.0], 1.0, 0.0, 50.0, 30.0),
+    (100, 23, 6, [0, 0, 1.0, 0, 0.5], 0.5, 0.0, 1e3, 200.0),
+    (130, 41, 10, [0, 0, 1.0, 0.8, 0.5], 0.7, 0.0, 1e2, 60.0),
+    (64, 9, 4, [0, 0, 0, 0.5, 0, 0, 0, 0, 0, 0.5], 0.3, 1.5, 40.0, 7.0),   # 3+9 model, beta0 > 0
+    (333, 301, 4, [0, 0, 2.0], 0.0, 0.0, 1e4, 900.0),                      # ragged L, pure 2-spin, T = 0
+    (48, 2, 2, [0, 0, 0, 1.0], 1.0, 0.0, 10.0, 0.01),                      # n_rows = 2: only row 0 + current row
+    (48, 3, 8, [0, 0, 0, 1.0], 1.0, 0.0, 10.0, 0.02),
+]
+
+
+@pytest.mark.parametrize("L,N,s,lam,T,beta0,t_max,t_end", CASES)
+def test_rhs_matches_oracle_small(D, L, N, s, lam, T, beta0, t_max, t_end):
+    ctx = D.dmfe_create(L, s, t_max, lam, T=T, beta0=beta0)
+    try:
+        tab = D.dmfe_get_tables(ctx, L)
+        grid = _oracle_grid_from_library(tab, L, s, t_max)
+        t, mu, hist = inputs.random_smooth_history(tab["theta"], tab["omega"], N, t_end, seed=L + N)
+        hist[N - 1, :, 1] = np.nan  # derivative slots of the current row must be ignored
+        hist[N - 1, :, 3] = np.inf
+        mu[N - 1] = np.nan
+        g = gpu_rhs(D, ctx, L, t, mu, hist, N)
+    finally:
+        D.dmfe_destroy(ctx)
+    model = O.Model(np.array(lam, dtype=np.float64), T, beta0)
+    ref = O.history_integrals(grid, model, t, mu, hist, N - 1, tables=(tab["start"], tab["frac"]), want_rows=True)
+    ref["theta"] = tab["theta"]
+    compare_rhs(g, ref)
+
+
+@pytest.mark.parametrize("L,lo,hi,t_max,lam", [
+    (512, -2.0, 4.0, 1e4, [0, 0, 0, 1.0]),                 # config-2 recipe at reduced L
+    (1024, -2.0, 7.0, 1e7, [0, 0, 1.0, 0.8, 0.5]),         # config-5 recipe, smallest L
+])
+def test_rhs_matches_oracle_synthetic(D, L, lo, hi, t_max, lam):
+    s = 4
+    ctx = D.dmfe_create(L, s, t_max, lam, T=0.5)
+    try:
+        tab = D.dmfe_get_tables(ctx, L)
+        grid = _oracle_grid_from_library(tab, L, s, t_max)
+        t, mu, hist = inputs.synthetic_history(tab["theta"], tab["omega"], L, lo, hi)
+        g = gpu_rhs(D, ctx, L, t, mu, hist, L)
+    finally:
+        D.dmfe_destroy(ctx)
+    model = O.Model(np.array(lam, dtype=np.float64), 0.5, 0.0)
+    ref = O.history_integrals(grid, model, t, mu, hist, L - 1, tables=(tab["start"], tab["frac"]), want_rows=True)
+    ref["theta"] = tab["theta"]
+    compare_rhs(g, ref)
+
+
+def test_rhs_rows_in_a_larger_buffer(D):
+    """n_rows < n_cap: rows beyond the current one are never touched (filled with NaN here)."""
+    L, N, s = 80, 20, 4
+    ctx = D.dmfe_create(L, s, 100.0, [0, 0, 0, 1.0], T=0.8)
+    try:
+        tab = D.dmfe_get_tables(ctx, L)
+        grid = _oracle_grid_from_library(tab, L, s, 100.0)
+        t, mu, hist = inputs.random_smooth_history(tab["theta"], tab["omega"], N, 12.0, seed=5)
+        cap = N + 7
+        t2 = np.full(cap, np.nan); t2[:N] = t
+        mu2 = np.full(cap, np.nan); mu2[:N] = mu
+        h2 = np.full((cap, L, 4), np.nan); h2[:N] = hist
+        g = gpu_rhs(D, ctx, L, t2, mu2, h2, N)
+    finally:
+        D.dmfe_destroy(ctx)
+    model = O.Model(np.array([0, 0, 0, 1.0]), 0.8, 0.0)
+    ref = O.history_integrals(grid, model, t, mu, hist, N - 1, tables=(tab["start"], tab["frac"]), want_rows=True)
+    ref["theta"] = tab["theta"]
+    compare_rhs(g, ref)
+
+
+def test_host_buffer_call_equals_device_call(D):
+    L, N, s = 96, 30, 4
+    ctx = D.dmfe_create(L, s, 100.0, [0, 0, 0, 1.0], T=0.8)
+    try:
+        tab = D.dmfe_get_tables(ctx, L, want_pairs=False)
+        t, mu, hist = inputs.random_smooth_history(tab["theta"], tab["omega"], N, 12.0, seed=6)
+        g = gpu_rhs(D, ctx, L, t, mu, hist, N, want_rows=False)
+        d1C, d1R, m, e = np.zeros(L), np.zeros(L), np.zeros(1), np.zeros(1)
+        D.dmfe_history_integrals_host(ctx, N, t, mu, hist, d1C, d1R, m, e)
+    finally:
+        D.dmfe_destroy(ctx)
+    assert np.array_equal(d1C, g["d1C"]) and np.array_equal(d1R, g["d1R"])
+    assert m[0] == g["mu_out"][0] and e[0] == g["energy"][0]
+
+
+def test_bad_arguments_are_rejected(D):
+    with pytest.raises(D.DmfeError):
+        D.dmfe_create(6, 4, 100.0, [0, 0, 0, 1.0], T=1.0)        # L < 2s
+    with pytest.raises(D.DmfeError):
+        D.dmfe_create(64, 5, 100.0, [0, 0, 0, 1.0], T=1.0)       # odd stencil
+    with pytest.raises(D.DmfeError):
+        D.dmfe_create(64, 4, 2.0, [0, 0, 0, 1.0], T=1.0)         # t_max <= e
+    import torch
+    ctx = D.dmfe_create(64, 4, 100.0, [0, 0, 0, 1.0], T=1.0)
+    try:
+        z = torch.zeros(4, dtype=torch.float64, device="cuda")
+        h = torch.zeros((4, 64, 4), dtype=torch.float64, device="cuda")
+        with pytest.raises(D.DmfeError):
+            D.dmfe_history_integrals(ctx, 1, z, z, h)              # n_rows < 2
+    finally:
+        D.dmfe_destroy(ctx)

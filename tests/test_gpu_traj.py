@@ -1,0 +1,186 @@
+"""GPU parity, Stage C: device-resident SSPRK(10,4) steps, controller and sparsification against
+the oracle's step-by-step implementation.
+
+Fixed-step trajectories: observables (E, mu, rows of C and R) within 1e-9 relative (north_star).
+Adaptive runs: accept/revert decisions and sparsification keep-masks bit-exact over the compared
+window; the oracle runs on the library's tables (theta, omega, nu, start, frac).
+"""
+import numpy as np
+import pytest
+
+from oracle import dmfe_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def D():
+    from paper_2604_06309_b200 import dmfe
+    dmfe.load_library()
+    return dmfe
+
+
+def _oracle_grid(D, ctx, L, s, t_max):
+    tab = D.dmfe_get_tables(ctx, L)
+    g = O.Grid(L=L, s=s, t_max=t_max, theta=tab["theta"], omega=tab["omega"], nu=tab["nu"])
+    g._tables = (tab["start"], tab["frac"])
+    return g
+
+
+def _pull(st, ten):
+    n = st.n_rows
+    return (ten["t"][:n].cpu().numpy(), ten["mu"][:n].cpu().numpy(), ten["energy"][:n].cpu().numpy(),
+            ten["hist"][:n].cpu().numpy())
+
+
+def _assert_traj_close(got, H, rtol):
+    t, mu, E, hist = got
+    n = H.n_rows
+    assert len(t) == n
+    np.testing.assert_allclose(t, H.t[:n], rtol=1e-14, atol=0)
+    np.testing.assert_allclose(mu, H.mu[:n], rtol=rtol, atol=0)
+    np.testing.assert_allclose(E, H.E[:n], rtol=rtol, atol=rtol * 1e-3)
+    # C and R rows: relative to the field scale 1 (values decay towards 0 away from the diagonal)
+    np.testing.assert_allclose(hist[:, :, 0], H.hist[:n, :, 0], rtol=rtol, atol=rtol)
+    np.testing.assert_allclose(hist[:, :, 2], H.hist[:n, :, 2], rtol=rtol, atol=rtol)
+    # stored ray derivatives
+    np.testing.assert_allclose(hist[:, :, 1], H.hist[:n, :, 1], rtol=rtol, atol=10 * rtol)
+    np.testing.assert_allclose(hist[:, :, 3], H.hist[:n, :, 3], rtol=rtol, atol=10 * rtol)
+
+
+@pytest.mark.parametrize("L,s,lam,T,beta0,h,steps", [
+    (64, 4, [0, 0, 0, 1.0], 1.0, 0.0, 0.05, 40),          # config 1 shape, shortened
+    (48, 6, [0, 0, 1.0, 0, 0.5], 0.5, 0.0, 0.02, 25),     # mixed 2+4
+    (40, 4, [0, 0, 0, 1.0], 0.8, 1.2, 0.03, 20),          # beta0 > 0 start
+])
+def test_fixed_step_trajectory(D, L, s, lam, T, beta0, h, steps):
+    t_max = 20.0
+    ctx = D.dmfe_create(L, s, t_max, lam, T=T, beta0=beta0)
+    try:
+        grid = _oracle_grid(D, ctx, L, s, t_max)
+        st, ten = D.make_state(L, steps + 3)
+        D.dmfe_init_state(ctx, st, h)
+        for _ in range(steps):
+            assert D.dmfe_rk_step(ctx, st, fixed_step=True)
+        got = _pull(st, ten)
+        assert st.n_rows == steps + 1 and st.n_rhs == 10 * steps
+    finally:
+        D.dmfe_destroy(ctx)
+    model = O.Model(np.array(lam, dtype=np.float64), T, beta0)
+    H = O.run_fixed(grid, model, h, steps)
+    _assert_traj_close(got, H, 1e-9)
+    # P6 on the GPU result itself: C(t,t) = 1 and R(t,t-) = 1 are preserved by the scheme
+    assert np.max(np.abs(got[3][:, -1, 0] - 1.0)) < 1e-13
+    assert np.max(np.abs(got[3][:, -1, 2] - 1.0)) < 1e-13
+
+
+def test_config1_paramagnet_full(D):
+    """BASELINE.json config 1: p=3, T=1, h=0.05 to t=20 (400 steps), L=128, s=4; oracle ~10 s."""
+    L, s, t_max, h, steps = 128, 4, 20.0, 0.05, 400
+    lam = [0, 0, 0, 1.0]
+    ctx = D.dmfe_create(L, s, t_max, lam, T=1.0)
+    try:
+        grid = _oracle_grid(D, ctx, L, s, t_max)
+        st, ten = D.make_state(L, steps + 3)
+        D.dmfe_init_state(ctx, st, h)
+        for _ in range(steps):
+            D.dmfe_rk_step(ctx, st, fixed_step=True)
+        got = _pull(st, ten)
+    finally:
+        D.dmfe_destroy(ctx)
+    H = O.run_fixed(grid, O.Model(np.array(lam, dtype=np.float64), 1.0, 0.0), h, steps)
+    _assert_traj_close(got, H, 1e-9)
+    t, mu, E, hist = got
+    # P7: paramagnet equilibrium mu -> T + f'(1)/T = 2.5, E -> -f(1)/T = -0.5
+    assert abs(mu[-1] - 2.5) < 2e-4 and abs(E[-1] + 0.5) < 1e-4
+
+
+def test_adaptive_decisions_and_sparsify_masks(D):
+    L, s, t_max, tol = 64, 4, 200.0, 1e-6
+    lam = [0, 0, 0, 1.0]
+    T = 0.5
+    n_cap, sp_every, protect = 400, 50, 12
+    n_steps = 260
+    ctx = D.dmfe_create(L, s, t_max, lam, T=T, tol=tol)
+    try:
+        grid = _oracle_grid(D, ctx, L, s, t_max)
+        st, ten = D.make_state(L, n_cap)
+        D.dmfe_init_state(ctx, st, 1e-3)
+        model = O.Model(np.array(lam, dtype=np.float64), T, 0.0)
+        H = O.History(grid, model, n_cap)
+        h = min(1e-3, O.h_stab(model))
+        acc = 0
+        for step in range(n_steps):
+            if acc > 0 and acc % sp_every == 0:
+                keep_ref, _ = O.sparsify(H, tol, protect)
+                n_after, keep = D.dmfe_sparsify(ctx, st, protect, want_mask=True)
+                assert np.array_equal(keep, keep_ref), "keep mask differs at step %d" % step
+                assert n_after == H.n_rows == st.n_rows
+                acc += 1
+            ok_ref, h, eps_ref = O.controller_step(H, h, tol)
+            ok = D.dmfe_rk_step(ctx, st)
+            assert ok == ok_ref, "accept/revert decision differs at step %d" % step
+            assert st.n_rows == H.n_rows
+            assert abs(st.h - h) <= 1e-15 * h
+            assert abs(st.eps_rk - eps_ref) <= 1e-6 * eps_ref + 1e-18
+            if ok:
+                acc += 1
+        got = _pull(st, ten)
+    finally:
+        D.dmfe_destroy(ctx)
+    _assert_traj_close(got, H, 1e-9)
+
+
+def test_revert_path(D):
+    """A step that is far too large must be rejected: rows dropped (at most 10), h halved."""
+    L, s = 48, 4
+    ctx = D.dmfe_create(L, s, 50.0, [0, 0, 0, 1.0], T=0.5, tol=1e-10)
+    try:
+        st2, ten2 = D.make_state(L, 64)
+        D.dmfe_init_state(ctx, st2, 1.5)      # h0 = 1.5 from t = 0: eps_RK >> tol
+        ok = D.dmfe_rk_step(ctx, st2)
+        assert not ok and st2.n_rows == 1 and abs(st2.h - 0.75) < 1e-15
+    finally:
+        D.dmfe_destroy(ctx)
+
+
+def test_capacity_error(D):
+    L = 32
+    ctx = D.dmfe_create(L, 4, 50.0, [0, 0, 0, 1.0], T=0.5)
+    try:
+        st, ten = D.make_state(L, 4)
+        D.dmfe_init_state(ctx, st, 1e-3)
+        for _ in range(3):
+            D.dmfe_rk_step(ctx, st, fixed_step=True)
+        with pytest.raises(D.DmfeError) as ei:
+            D.dmfe_rk_step(ctx, st, fixed_step=True)
+        assert ei.value.code == D.DMFE_ECAPACITY
+    finally:
+        D.dmfe_destroy(ctx)
+
+
+def test_sparsify_on_synthetic_rows(D):
+    """Sparsify alone on a seeded smooth history: keep mask, compacted t/mu/rows bit-exact."""
+    import torch
+    from paper_2604_06309_b200 import inputs
+    L, N, s, tol = 72, 90, 4, 0.015
+    ctx = D.dmfe_create(L, s, 100.0, [0, 0, 0, 1.0], T=0.5, tol=tol)
+    try:
+        tab = D.dmfe_get_tables(ctx, L, want_pairs=False)
+        t, mu, hist = inputs.random_smooth_history(tab["theta"], tab["omega"], N, 3.0, seed=11)
+        st, ten = D.make_state(L, N + 5)
+        ten["t"][:N] = torch.from_numpy(t).cuda()
+        ten["mu"][:N] = torch.from_numpy(mu).cuda()
+        ten["hist"][:N] = torch.from_numpy(hist).cuda()
+        st.n_rows = N
+        n_after, keep = D.dmfe_sparsify(ctx, st, 12, want_mask=True)
+        got = _pull(st, ten)
+    finally:
+        D.dmfe_destroy(ctx)
+    eps = O.sparsify_residuals(L, N, t, hist)
+    keep_ref = O.sparsify_mask(eps, N, tol, 12)
+    assert 0 < (~keep_ref).sum() < N - 13, "test must drop some but not all rows"
+    assert np.array_equal(keep, keep_ref)
+    assert n_after == keep_ref.sum()
+    assert np.array_equal(got[0], t[keep_ref]) and np.array_equal(got[1], mu[keep_ref])
+    assert np.array_equal(got[3], hist[keep_ref])
