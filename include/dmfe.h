@@ -149,6 +149,10 @@ DMFE_API int dmfe_sparsify(dmfe_ctx *ctx, dmfe_state *st, int32_t protect_last, 
  * 2*DFMA/s: the denominator of the FP64 roofline, measured rather than assumed. */
 DMFE_API int dmfe_enable_timing(dmfe_ctx *ctx, int32_t on);
 DMFE_API int dmfe_last_kernel_ms(dmfe_ctx *ctx, float *ms);
+/* Sum (and minimum) of the pair-kernel durations of all launches since timing was switched on
+ * (at most 512 are kept); synchronises on the last one.  No synchronisation happens between the
+ * launches themselves, so this can bracket every launch of a timed region. */
+DMFE_API int dmfe_kernel_time_stats(dmfe_ctx *ctx, int32_t *n_launches, double *total_ms, double *min_ms);
 DMFE_API int dmfe_probe_fp64_tflops(dmfe_ctx *ctx, int32_t n_iter, double *tflops, int32_t *sm_count);
 
 #ifdef __cplusplus

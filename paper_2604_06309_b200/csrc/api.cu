@@ -43,8 +43,7 @@ static void free_all(dmfe_ctx *c) {
   cudaFree(c->stage_mu);
   cudaFree(c->stage_hist);
   cudaFree(c->stage_out);
-  if (c->ev0) cudaEventDestroy(c->ev0);
-  if (c->ev1) cudaEventDestroy(c->ev1);
+  for (int k = 0; k < 2 * c->ev_made; ++k) cudaEventDestroy(c->ev[k]);
   if (c->h_scal) cudaFreeHost(c->h_scal);
   if (c->h_iscal) cudaFreeHost(c->h_iscal);
 }
@@ -85,8 +84,6 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
     if (e == cudaSuccess) e = cudaMalloc(&c->rk, sizeof(double) * 8 * (size_t)L);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_scal, sizeof(double) * SC_COUNT);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_iscal, sizeof(int32_t) * IS_COUNT);
-    if (e == cudaSuccess) e = cudaEventCreate(&c->ev0);
-    if (e == cudaSuccess) e = cudaEventCreate(&c->ev1);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->scal, 0, sizeof(double) * SC_COUNT, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->iscal, 0, sizeof(int32_t) * IS_COUNT, c->stream);
     if (e != cudaSuccess) {

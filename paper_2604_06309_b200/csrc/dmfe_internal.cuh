@@ -6,6 +6,7 @@
 #include "dmfe.h"
 
 #define DMFE_PMAX_MAX 15
+#define DMFE_EV_RING 512
 
 // f(q) = 1/2 sum_p lambda_p q^p (Eq.(4)).  Horner coefficients, lowest power first:
 //   f (q) = sum_k c0[k] q^k        c0[k] = lambda_k / 2
@@ -65,7 +66,9 @@ struct dmfe_ctx {
   int32_t stage_rows;
   // measurement hooks
   int timing_on;
-  cudaEvent_t ev0, ev1;
+  cudaEvent_t ev[2 * DMFE_EV_RING];  // (before, after) pairs around the pair kernel, lazily created
+  int ev_made;                       // pairs created so far
+  int ev_n;                          // pairs recorded since timing was switched on
   // pinned host scalars for the one-record-per-step readback
   double *h_scal;
   int32_t *h_iscal;

@@ -313,7 +313,15 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, const double *t, const double *mu_
   a.cur = ctx->cur;
   a.scal = ctx->scal;
   a.out = *out;
-  if (ctx->timing_on) CUDA_TRY(ctx, cudaEventRecord(ctx->ev0, ctx->stream));
+  const bool timed = ctx->timing_on && ctx->ev_n < DMFE_EV_RING;
+  if (timed) {
+    if (ctx->ev_n >= ctx->ev_made) {
+      CUDA_TRY(ctx, cudaEventCreate(&ctx->ev[2 * ctx->ev_made]));
+      CUDA_TRY(ctx, cudaEventCreate(&ctx->ev[2 * ctx->ev_made + 1]));
+      ctx->ev_made++;
+    }
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev[2 * ctx->ev_n], ctx->stream));
+  }
   switch (ctx->p.stencil) {
     case 2: history_integrals_kernel<2><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
     case 4: history_integrals_kernel<4><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
@@ -322,7 +330,10 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, const double *t, const double *mu_
     case 10: history_integrals_kernel<10><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
     default: return DMFE_EINVAL;
   }
-  if (ctx->timing_on) CUDA_TRY(ctx, cudaEventRecord(ctx->ev1, ctx->stream));
+  if (timed) {
+    CUDA_TRY(ctx, cudaEventRecord(ctx->ev[2 * ctx->ev_n + 1], ctx->stream));
+    ctx->ev_n++;
+  }
   CUDA_TRY(ctx, cudaGetLastError());
   return DMFE_OK;
 }

@@ -30,13 +30,31 @@ extern "C" {
 int dmfe_enable_timing(dmfe_ctx *ctx, int32_t on) {
   if (!ctx) return DMFE_EINVAL;
   ctx->timing_on = on ? 1 : 0;
+  ctx->ev_n = 0;
   return DMFE_OK;
 }
 
 int dmfe_last_kernel_ms(dmfe_ctx *ctx, float *ms) {
-  if (!ctx || !ms || !ctx->timing_on) return DMFE_EINVAL;
-  CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev1));
-  CUDA_TRY(ctx, cudaEventElapsedTime(ms, ctx->ev0, ctx->ev1));
+  if (!ctx || !ms || ctx->ev_n < 1) return DMFE_EINVAL;
+  const int k = ctx->ev_n - 1;
+  CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev[2 * k + 1]));
+  CUDA_TRY(ctx, cudaEventElapsedTime(ms, ctx->ev[2 * k], ctx->ev[2 * k + 1]));
+  return DMFE_OK;
+}
+
+int dmfe_kernel_time_stats(dmfe_ctx *ctx, int32_t *n_launches, double *total_ms, double *min_ms) {
+  if (!ctx || !n_launches || !total_ms) return DMFE_EINVAL;
+  double tot = 0.0, mn = 1e300;
+  for (int k = 0; k < ctx->ev_n; ++k) {
+    float ms = 0.f;
+    CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev[2 * k + 1]));
+    CUDA_TRY(ctx, cudaEventElapsedTime(&ms, ctx->ev[2 * k], ctx->ev[2 * k + 1]));
+    tot += (double)ms;
+    if ((double)ms < mn) mn = (double)ms;
+  }
+  *n_launches = ctx->ev_n;
+  *total_ms = tot;
+  if (min_ms) *min_ms = ctx->ev_n ? mn : 0.0;
   return DMFE_OK;
 }
 

@@ -19,7 +19,8 @@ DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE
 
 EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror", "dmfe_get_tables",
            "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_init_state", "dmfe_rk_step",
-           "dmfe_sparsify", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_probe_fp64_tflops"]
+           "dmfe_sparsify", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
+           "dmfe_probe_fp64_tflops"]
 
 
 class dmfe_params(Structure):
@@ -84,6 +85,8 @@ def load_library():
     lib.dmfe_enable_timing.argtypes = [c_void_p, c_int32]
     lib.dmfe_last_kernel_ms.restype = c_int
     lib.dmfe_last_kernel_ms.argtypes = [c_void_p, POINTER(ctypes.c_float)]
+    lib.dmfe_kernel_time_stats.restype = c_int
+    lib.dmfe_kernel_time_stats.argtypes = [c_void_p, POINTER(c_int32), POINTER(c_double), POINTER(c_double)]
     lib.dmfe_probe_fp64_tflops.restype = c_int
     lib.dmfe_probe_fp64_tflops.argtypes = [c_void_p, c_int32, POINTER(c_double), POINTER(c_int32)]
     _lib = lib
@@ -209,6 +212,13 @@ def dmfe_last_kernel_ms(ctx):
     ms = ctypes.c_float(0.0)
     _check(load_library().dmfe_last_kernel_ms(ctx, byref(ms)), "dmfe_last_kernel_ms", ctx)
     return float(ms.value)
+
+
+def dmfe_kernel_time_stats(ctx):
+    """-> (launches timed, total ms, min ms) of the pair kernel since dmfe_enable_timing(True)"""
+    n, tot, mn = c_int32(0), c_double(0.0), c_double(0.0)
+    _check(load_library().dmfe_kernel_time_stats(ctx, byref(n), byref(tot), byref(mn)), "dmfe_kernel_time_stats", ctx)
+    return n.value, tot.value, mn.value
 
 
 def dmfe_probe_fp64_tflops(ctx, n_iter=1 << 16):
