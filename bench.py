@@ -307,7 +307,7 @@ def run_ours(args):
         samp = np.arange(0, L, max(1, L // 512))
         cells, sampled = unique_cells(theta, omega, t, s, L, N, sample=samp), True
     alg_bytes = 32 * cells + 8 * 8 * L
-    table_bytes = 36 * pairs
+    table_bytes = 24 * pairs
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))

@@ -29,8 +29,9 @@ static void free_all(dmfe_ctx *c) {
   cudaFree(c->theta);
   cudaFree(c->omega);
   cudaFree(c->nu);
-  cudaFree(c->start);
-  cudaFree(c->frac);
+  cudaFree(c->tab);
+  cudaFree(c->blo);
+  cudaFree(c->rowtab);
   cudaFree(c->cur);
   cudaFree(c->scal);
   cudaFree(c->iscal);
@@ -79,6 +80,7 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
   if (rc == DMFE_OK) {
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&c->cur, sizeof(double2) * (size_t)L);
+    if (e == cudaSuccess) e = cudaMalloc(&c->blo, sizeof(int32_t) * (size_t)L);
     if (e == cudaSuccess) e = cudaMalloc(&c->scal, sizeof(double) * SC_COUNT);
     if (e == cudaSuccess) e = cudaMalloc(&c->iscal, sizeof(int32_t) * IS_COUNT);
     if (e == cudaSuccess) e = cudaMalloc(&c->rk, sizeof(double) * 8 * (size_t)L);
@@ -119,14 +121,26 @@ int dmfe_get_tables(dmfe_ctx *ctx, double *theta, double *omega, double *nu, int
   if (start || frac) {
     if (i0 < 0 || n_targets < 1 || i0 + n_targets > L) return DMFE_EINVAL;
     const size_t plane = (size_t)L * (size_t)L, blk = (size_t)n_targets * (size_t)L;
+    uint64_t *tmp = (uint64_t *)malloc(blk * sizeof(uint64_t));
+    if (!tmp) return DMFE_ENOMEM;
     for (int k = 0; k < 3; ++k) {
-      if (start)
-        CUDA_TRY(ctx, cudaMemcpyAsync(start + k * blk, ctx->start + k * plane + (size_t)i0 * L,
-                                      blk * sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
-      if (frac)
-        CUDA_TRY(ctx, cudaMemcpyAsync(frac + k * blk, ctx->frac + k * plane + (size_t)i0 * L,
-                                      blk * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+      cudaError_t e = cudaMemcpyAsync(tmp, ctx->tab + k * plane + (size_t)i0 * L, blk * sizeof(uint64_t),
+                                      cudaMemcpyDeviceToHost, ctx->stream);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+      if (e != cudaSuccess) {
+        free(tmp);
+        ctx->cuda_err = (int)e;
+        return DMFE_ECUDA;
+      }
+      for (size_t q = 0; q < blk; ++q) {  // decode: exactly the values the pair kernel uses
+        int32_t st;
+        double fr;
+        dmfe_tab_decode(tmp[q], &st, &fr);
+        if (start) start[k * blk + q] = st;
+        if (frac) frac[k * blk + q] = fr;
+      }
     }
+    free(tmp);
   }
   CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
   return DMFE_OK;
@@ -135,7 +149,7 @@ int dmfe_get_tables(dmfe_ctx *ctx, double *theta, double *omega, double *nu, int
 int dmfe_history_integrals(dmfe_ctx *ctx, const dmfe_grid *g, const dmfe_rhs_out *out) {
   if (!ctx || !g || !out) return DMFE_EINVAL;
   if (g->n_rows < 2 || g->n_rows > g->n_cap || !g->t || !g->mu || !g->hist) return DMFE_EINVAL;
-  return dmfe_launch_rhs(ctx, g->n_rows - 1, g->t, g->mu, g->hist, out);
+  return dmfe_launch_rhs(ctx, g->n_rows - 1, g->n_cap, g->t, g->mu, g->hist, out);
 }
 
 int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const double *t, const double *mu_hist,
@@ -166,7 +180,7 @@ int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const double *t, 
   o.d1R = ctx->stage_out + L;
   o.mu = ctx->stage_out + 2 * L;
   o.energy = ctx->stage_out + 2 * L + 1;
-  const int rc = dmfe_launch_rhs(ctx, n_rows - 1, ctx->stage_t, ctx->stage_mu, ctx->stage_hist, &o);
+  const int rc = dmfe_launch_rhs(ctx, n_rows - 1, n_rows, ctx->stage_t, ctx->stage_mu, ctx->stage_hist, &o);
   if (rc != DMFE_OK) return rc;
   if (d1C) CUDA_TRY(ctx, cudaMemcpyAsync(d1C, o.d1C, sizeof(double) * (size_t)L, cudaMemcpyDeviceToHost, s));
   if (d1R) CUDA_TRY(ctx, cudaMemcpyAsync(d1R, o.d1R, sizeof(double) * (size_t)L, cudaMemcpyDeviceToHost, s));

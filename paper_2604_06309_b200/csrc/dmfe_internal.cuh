@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include "dmfe.h"
 
@@ -48,10 +49,12 @@ struct dmfe_ctx {
   double h_stab;       // 13.9 / (4 sqrt(f''(1)))  (Eq.(24))
   // ---- tables (device) ----
   double *theta, *omega, *nu;  // [L]
-  int32_t *start;              // [3][L][L]
-  double *frac;                // [3][L][L]
+  uint64_t *tab;               // [3][L][L] packed {stencil start : 16 | fractional coordinate : 48}
   // ---- O(L) scratch (device) ----
   double2 *cur;     // [L] {C, R} of the current row, packed for 16-byte gathers
+  int32_t *blo;     // [L] per-call row bracket table: blo[c] = n(theta_c t_M)
+  double2 *rowtab;  // [rowtab_cap] per-call {t_n, t_{n+1} - t_n}
+  int32_t rowtab_cap;
   double *scal;     // [SC_COUNT]
   int32_t *iscal;   // [IS_COUNT]
   double *rk;       // [4][L][2]: q1, q2, delta, F
@@ -83,8 +86,37 @@ struct dmfe_ctx {
     }                                                    \
   } while (0)
 
+// Packed pair-table entry: bits 63..48 = stencil start (L <= 65535), bits 47..0 = the fractional
+// index coordinate u = X - start in fixed point: q = rint((u + 17) 2^44) - 2^48, i.e. the top 48
+// mantissa bits of the double u + 17 in [16, 32) (resolution 2^-44 = 5.7e-14 index units, far
+// below the ~4e-12 accuracy of X itself in fp64; -1 < u < 15 covers every stencil, s <= 10).
+// The decoded value is THE coordinate of the library: dmfe_get_tables returns it.
+#if defined(__CUDACC__)
+#define DMFE_HD __host__ __device__ __forceinline__
+#else
+#define DMFE_HD inline
+#endif
+DMFE_HD uint64_t dmfe_tab_encode(int32_t start, double frac) {
+  const double x = (frac + 17.0) * 17592186044416.0;  // 2^44: exact scaling
+  long long q = (long long)rint(x) - (16LL << 44);
+  if (q < 0) q = 0;
+  if (q > (1LL << 48) - 1) q = (1LL << 48) - 1;
+  return ((uint64_t)(uint32_t)start << 48) | (uint64_t)q;
+}
+DMFE_HD void dmfe_tab_decode(uint64_t e, int32_t *start, double *frac) {
+  *start = (int32_t)(e >> 48);
+  const uint64_t bits = 0x4030000000000000ULL | ((e & 0xFFFFFFFFFFFFULL) << 4);
+  double x;
+#if defined(__CUDA_ARCH__)
+  x = __longlong_as_double((long long)bits);
+#else
+  memcpy(&x, &bits, sizeof(x));
+#endif
+  *frac = x - 17.0;
+}
+
 // tables.cu
 int dmfe_build_tables(dmfe_ctx *ctx);
 // history_integrals.cu
-int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, const double *t, const double *mu_hist, const double *hist,
-                    const dmfe_rhs_out *out);
+int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, const double *mu_hist,
+                    const double *hist, const dmfe_rhs_out *out);

@@ -13,21 +13,29 @@
 // read coalesced; the type-2 cells of adjacent lanes are neighbours in the packed history).
 // Every history cell {C,dC,R,dR} is one 256-bit load.  fp64 throughout; no tensor cores: every
 // "matrix" here is a gather.
+//
+// Launch 1 (prepare_kernel, O(L + M)): packs row M into {C,R} pairs, reduces mu and E, builds the
+// per-call row table {t_n, t_{n+1}-t_n} and the row bracket table blo[c] = n(theta_c t_M).
+// Launch 2 (history_integrals_kernel): the L^2 pairs.  The row search of a pair is
+// a bisection inside the bracket [blo[a], blo[b]] given by the grid cells a <= phi2 < b that the
+// phi2 stencil start already identifies -- same predicate and same result as a full bisection.
 #include "dmfe_internal.cuh"
 
 namespace {
 
 constexpr int RHS_THREADS = 256;
+constexpr int PREP_THREADS = 1024;
 
 struct RhsArgs {
   int32_t L, M;
   const double *theta, *omega, *nu;
-  const int32_t *start;
-  const double *frac;
+  const uint64_t *tab;
   const double *t, *mu_hist;
   const double4 *hist;
   const double2 *cur;
-  const double *scal;  // SC_MU, SC_E written by pack_mu_energy_kernel
+  const double2 *rowtab;
+  const int32_t *blo;
+  const double *scal;  // SC_MU, SC_E written by prepare_kernel
   dmfe_rhs_out out;
 };
 
@@ -37,6 +45,11 @@ __device__ __forceinline__ double4 ld_cell(const double4 *p) {
                : "=d"(v.x), "=d"(v.y), "=d"(v.z), "=d"(v.w)
                : "l"(p));
   return v;
+}
+
+// streamed once per call: keep it out of L1 and first in line for L2 eviction
+__device__ __forceinline__ uint64_t ld_stream(const uint64_t *p) {
+  return (uint64_t)__ldcs((const unsigned long long *)p);
 }
 
 __device__ __forceinline__ double horner(const double *c, int deg, double q) {
@@ -68,9 +81,8 @@ __device__ __forceinline__ void lagrange_weights(double u, double (&w)[S]) {
   }
 }
 
-// n = max{ n <= M-1 : t[n] <= tau }; t ascending, t[0] = 0 <= tau.
-__device__ __forceinline__ int row_search(const double *__restrict__ t, int M, double tau) {
-  int lo = 0, hi = M - 1;
+// n = max{ n in [lo, hi] : t[n] <= tau }; requires t[lo] <= tau.
+__device__ __forceinline__ int row_search(const double *__restrict__ t, int lo, int hi, double tau) {
   while (lo < hi) {
     const int mid = lo + ((hi - lo + 1) >> 1);
     if (__ldg(t + mid) <= tau)
@@ -83,32 +95,52 @@ __device__ __forceinline__ int row_search(const double *__restrict__ t, int M, d
 
 // weights of the local interpolant in t between rows n and n+1 (PAPER.md:260 cubic Hermite);
 // quadratic (value, slope, value) when the upper row is the current row M (reading G12).
-__device__ __forceinline__ void t_weights(double tn, double tn1, double tau, bool top, double (&h)[4]) {
-  const double D = tn1 - tn;
+//   h00 = 2u^3-3u^2+1, h10 = u(u-1)^2 D, h01 = 1-h00, h11 = u^2(u-1) D;  top: 1-u^2, u(1-u) D, u^2, 0
+__device__ __forceinline__ void t_weights(double tn, double D, double tau, bool top, double (&h)[4]) {
   const double u = (tau - tn) / D;
+  const double v = u - 1.0;
   const double u2 = u * u;
+  const double uvD = u * v * D;
   if (top) {
     h[0] = 1.0 - u2;
-    h[1] = (u - u2) * D;
+    h[1] = -uvD;
     h[2] = u2;
     h[3] = 0.0;
   } else {
-    const double u3 = u2 * u;
-    h[0] = 2.0 * u3 - 3.0 * u2 + 1.0;
-    h[1] = (u3 - 2.0 * u2 + u) * D;
-    h[2] = 3.0 * u2 - 2.0 * u3;
-    h[3] = (u3 - u2) * D;
+    h[0] = fma(u2, fma(2.0, u, -3.0), 1.0);
+    h[1] = uvD * v;
+    h[2] = 1.0 - h[0];
+    h[3] = uvD * u;
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// O(L) pre-pass: pack row M into {C,R} pairs and reduce mu(t) (Eq.(13)) and E(t) (Eq.(14)).
-__global__ void __launch_bounds__(1024) pack_mu_energy_kernel(int L, int M, ModelCoef mc,
-                                                              const double *__restrict__ nu,
-                                                              const double *__restrict__ t,
-                                                              const double4 *__restrict__ hist,
-                                                              double2 *__restrict__ cur,
-                                                              double *__restrict__ scal) {
+// O(L + M) pre-pass.  Block 0: pack row M into {C,R} pairs and reduce mu(t) (Eq.(13)) and E(t)
+// (Eq.(14)).  Blocks >= 1 (or block 0 too when launched alone): the per-call row table
+// rowtab[n] = {t_n, t_{n+1} - t_n}, n < M, and the bracket table blo[c] = n(fl(theta_c t_M)):
+// for theta_a <= phi < theta_b rounding is monotone, so n(fl(phi t_M)) lies in [blo[a], blo[b]].
+__global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, ModelCoef mc,
+                                                               const double *__restrict__ theta,
+                                                               const double *__restrict__ nu,
+                                                               const double *__restrict__ t,
+                                                               const double4 *__restrict__ hist,
+                                                               double2 *__restrict__ cur, double2 *__restrict__ rowtab,
+                                                               int32_t *__restrict__ blo, double *__restrict__ scal) {
+  if (blockIdx.x > 0 || gridDim.x == 1) {
+    const int nb = gridDim.x == 1 ? 1 : gridDim.x - 1;
+    const int b = gridDim.x == 1 ? 0 : blockIdx.x - 1;
+    const double tM = t[M];
+    for (int e = b * PREP_THREADS + threadIdx.x; e < M + L; e += nb * PREP_THREADS) {
+      if (e < M) {
+        const double tn = t[e];
+        rowtab[e] = make_double2(tn, t[e + 1] - tn);
+      } else {
+        const int c = e - M;
+        blo[c] = row_search(t, 0, M - 1, __dmul_rn(theta[c], tM));
+      }
+    }
+    if (blockIdx.x > 0) return;
+  }
   __shared__ double sm[32], se[32];
   const double4 *row = hist + (size_t)M * (size_t)L;
   double am = 0.0, ae = 0.0;
@@ -139,21 +171,24 @@ __global__ void __launch_bounds__(1024) pack_mu_energy_kernel(int L, int M, Mode
 
 // ---------------------------------------------------------------------------------------------
 template <int S>
-__global__ void __launch_bounds__(RHS_THREADS) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
+__global__ void __launch_bounds__(RHS_THREADS, 3) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
   const int L = a.L, M = a.M;
   const int i = blockIdx.x;
   const size_t plane = (size_t)L * (size_t)L;
-  const size_t rowoff = (size_t)i * (size_t)L;
+  const uint64_t *tab1 = a.tab + (size_t)i * (size_t)L, *tab2 = tab1 + plane, *tab3 = tab2 + plane;
   const double th_i = a.theta[i], om_i = a.omega[i];
   const double tM = a.t[M];
   const int d1 = mc.pmax - 1, d2 = mc.pmax - 2;
 
-  // type-1: one row search per target, tau = theta_i t  (Eq.(19))
+  // type-1: one row search per target, tau = theta_i t  (Eq.(19)); blo[i] is exactly that row
   const double tau1 = __dmul_rn(th_i, tM);
-  const int n1 = row_search(a.t, M, tau1);
+  const int n1 = a.blo[i];
   const bool top1 = (n1 + 1 == M);
   double h1[4];
-  t_weights(a.t[n1], a.t[n1 + 1], tau1, top1, h1);
+  {
+    const double2 rt = a.rowtab[n1];
+    t_weights(rt.x, rt.y, tau1, top1, h1);
+  }
   const double4 *row1lo = a.hist + (size_t)n1 * (size_t)L;
   const double4 *row1hi = row1lo + L;
 
@@ -164,19 +199,37 @@ __global__ void __launch_bounds__(RHS_THREADS) history_integrals_kernel(RhsArgs 
   __shared__ double b1c_first;
 
   for (int j = threadIdx.x; j < L; j += RHS_THREADS) {
-    const size_t e = rowoff + (size_t)j;
-    const int a1 = __ldg(a.start + e), a2 = __ldg(a.start + plane + e), a3 = __ldg(a.start + 2 * plane + e);
-    const double u1 = __ldg(a.frac + e), u2 = __ldg(a.frac + plane + e), u3 = __ldg(a.frac + 2 * plane + e);
+    const uint64_t e1 = ld_stream(tab1 + j), e2 = ld_stream(tab2 + j), e3 = ld_stream(tab3 + j);
+    const double nj = a.nu[j];
+    int a1, a2, a3;
+    double u1, u2, u3;
+    dmfe_tab_decode(e1, &a1, &u1);
+    dmfe_tab_decode(e2, &a2, &u2);
+    dmfe_tab_decode(e3, &a3, &u3);
     double w[S];
-    // ---- A factors on the current row (Eq.(18)) ----
-    double C1 = 0.0, R1 = 0.0, C2 = 0.0, R2 = 0.0;
-    lagrange_weights<S>(u1, w);
+    // ---- A factors at phi1 (Eq.(18)) and the type-1 lookup (Eq.(19)): sums S1, S3, S5, S6 ----
+    {
+      double C1 = 0.0, R1 = 0.0;
+      lagrange_weights<S>(u1, w);
 #pragma unroll
-    for (int l = 0; l < S; ++l) {
-      const double2 v = __ldg(a.cur + a1 + l);
-      C1 = fma(w[l], v.x, C1);
-      R1 = fma(w[l], v.y, R1);
+      for (int l = 0; l < S; ++l) {
+        const double2 v = __ldg(a.cur + a1 + l);
+        C1 = fma(w[l], v.x, C1);
+        R1 = fma(w[l], v.y, R1);
+      }
+      const double4 lo = ld_cell(row1lo + j);
+      double4 hi = ld_cell(row1hi + j);
+      if (top1) hi.y = 0.0, hi.w = 0.0;
+      const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
+      const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
+      if (j == 0) b1c_first = B1C;
+      acc[0] = fma(nj * (horner(mc.c2, d2, C1) * R1), B1C, acc[0]);   // S1: K(t,s) C(t',s)
+      acc[2] = fma(nj * horner(mc.c1, d1, C1), B1R, acc[2]);          // S3: D(t,s) R(t',s)
+      acc[4] = fma(nj * (horner(mc.c2, d2, B1C) * B1R), C1, acc[4]);  // S5: K(t',s) C(t,s)
+      acc[5] = fma(nj * horner(mc.c1, d1, B1C), R1, acc[5]);          // S6: D(t',s) R(t,s)
     }
+    // ---- A factors at phi2 (Eq.(18)) ----
+    double C2 = 0.0, R2 = 0.0;
     lagrange_weights<S>(u2, w);
 #pragma unroll
     for (int l = 0; l < S; ++l) {
@@ -184,22 +237,19 @@ __global__ void __launch_bounds__(RHS_THREADS) history_integrals_kernel(RhsArgs 
       C2 = fma(w[l], v.x, C2);
       R2 = fma(w[l], v.y, R2);
     }
-    // ---- type-1 lookup (Eq.(19)) ----
-    const double4 lo = ld_cell(row1lo + j);
-    double4 hi = ld_cell(row1hi + j);
-    if (top1) hi.y = 0.0, hi.w = 0.0;
-    const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
-    const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
-    if (j == 0) b1c_first = B1C;
-    // ---- type-2 lookup (Eq.(20)): theta-stencil first, then t ----
-    const double th_j = a.theta[j];
-    const double phi2 = __dadd_rn(th_i, __dmul_rn(om_i, th_j));
+    // ---- type-2 lookup (Eq.(20)): row search in the bracket of the phi2 grid cells ----
+    const double phi2 = __dadd_rn(th_i, __dmul_rn(om_i, a.theta[j]));
     const double tau2 = __dmul_rn(phi2, tM);
-    const int n2 = row_search(a.t, M, tau2);
-    if (a.out.rows2) a.out.rows2[e] = n2;
+    const int chi = (a2 == L - S) ? L - 1 : a2 + S / 2;
+    const int n2 = row_search(a.t, __ldg(a.blo + a2), __ldg(a.blo + chi), tau2);
+    if (a.out.rows2) a.out.rows2[(size_t)i * (size_t)L + (size_t)j] = n2;
     const bool top2 = (n2 + 1 == M);
     double h2[4];
-    t_weights(__ldg(a.t + n2), __ldg(a.t + n2 + 1), tau2, top2, h2);
+    {
+      const double2 rt = __ldg(a.rowtab + n2);
+      t_weights(rt.x, rt.y, tau2, top2, h2);
+    }
+    // theta-stencil first, then t
     lagrange_weights<S>(u3, w);
     const double4 *p2 = a.hist + (size_t)n2 * (size_t)L + a3;
     double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
@@ -219,20 +269,14 @@ __global__ void __launch_bounds__(RHS_THREADS) history_integrals_kernel(RhsArgs 
     if (top2) dcu = 0.0, dru = 0.0;
     const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
     const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
-    // ---- kernel functions (Eq.(10)-(11)) and the eight terms (Eq.(21)) ----
-    const double nj = a.nu[j];
-    const double K1 = nj * (horner(mc.c2, d2, C1) * R1);
-    const double K2 = nj * (horner(mc.c2, d2, C2) * R2);
-    acc[0] = fma(K1, B1C, acc[0]);                                   // S1: K(t,s) C(t',s)
+    // ---- kernel functions (Eq.(10)-(11)) and the type-2 terms (Eq.(21)) ----
+    const double nR2 = nj * R2;
+    const double K2 = horner(mc.c2, d2, C2) * nR2;
     acc[1] = fma(K2, B2C, acc[1]);                                   // S2: K(t,s) C(s,t')
-    acc[2] = fma(nj * horner(mc.c1, d1, C1), B1R, acc[2]);           // S3: D(t,s) R(t',s)
     acc[3] = fma(K2, B2R, acc[3]);                                   // S4: K(t,s) R(s,t')
-    acc[4] = fma(nj * (horner(mc.c2, d2, B1C) * B1R), C1, acc[4]);   // S5: K(t',s) C(t,s)
-    acc[5] = fma(nj * horner(mc.c1, d1, B1C), R1, acc[5]);           // S6: D(t',s) R(t,s)
-    acc[6] = fma(nj * horner(mc.c1, d1, B2C), R2, acc[6]);           // S7: D(s,t') R(t,s)
-    acc[7] = fma(nj * R2, horner(mc.c2, d2, B2C) * B2R, acc[7]);     // S8: R(t,s) K(s,t')
+    acc[6] = fma(horner(mc.c1, d1, B2C), nR2, acc[6]);               // S7: D(s,t') R(t,s)
+    acc[7] = fma(nR2, horner(mc.c2, d2, B2C) * B2R, acc[7]);         // S8: R(t,s) K(s,t')
   }
-
   // ---- reduction over j: shuffle within the warp, fixed order across warps ----
 #pragma unroll
   for (int k = 0; k < 8; ++k)
@@ -294,23 +338,36 @@ __global__ void __launch_bounds__(RHS_THREADS) history_integrals_kernel(RhsArgs 
 }  // namespace
 
 // M = index of the current row; its time t[M] is read on the device (the RK step keeps t there).
-int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, const double *t, const double *mu_hist, const double *hist,
-                    const dmfe_rhs_out *out) {
+int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, const double *mu_hist,
+                    const double *hist, const dmfe_rhs_out *out) {
   const int L = ctx->p.L;
-  pack_mu_energy_kernel<<<1, 1024, 0, ctx->stream>>>(L, M, ctx->model, ctx->nu, t, (const double4 *)hist,
-                                                     ctx->cur, ctx->scal);
+  if (M > ctx->rowtab_cap) {  // per-call row table: sized by the caller's capacity, grown on demand
+    const int cap = n_cap > M ? n_cap : M;
+    CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->rowtab);
+    ctx->rowtab = nullptr;
+    ctx->rowtab_cap = 0;
+    CUDA_TRY(ctx, cudaMalloc(&ctx->rowtab, sizeof(double2) * (size_t)cap));
+    ctx->rowtab_cap = cap;
+  }
+  int pb = 1 + (M + L + PREP_THREADS - 1) / PREP_THREADS;
+  if (pb > 17) pb = 17;
+  prepare_kernel<<<pb, PREP_THREADS, 0, ctx->stream>>>(L, M, ctx->model, ctx->theta, ctx->nu, t,
+                                                       (const double4 *)hist, ctx->cur, ctx->rowtab, ctx->blo,
+                                                       ctx->scal);
   RhsArgs a;
   a.L = L;
   a.M = M;
   a.theta = ctx->theta;
   a.omega = ctx->omega;
   a.nu = ctx->nu;
-  a.start = ctx->start;
-  a.frac = ctx->frac;
+  a.tab = ctx->tab;
   a.t = t;
   a.mu_hist = mu_hist;
   a.hist = (const double4 *)hist;
   a.cur = ctx->cur;
+  a.rowtab = ctx->rowtab;
+  a.blo = ctx->blo;
   a.scal = ctx->scal;
   a.out = *out;
   const bool timed = ctx->timing_on && ctx->ev_n < DMFE_EV_RING;

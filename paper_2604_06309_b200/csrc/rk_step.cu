@@ -161,7 +161,7 @@ int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *acc
   o.F = F;
   for (int k = 0; k < 10; ++k) {
     if (k > 0) {
-      const int rc = dmfe_launch_rhs(ctx, M, st->t, st->mu, st->hist, &o);
+      const int rc = dmfe_launch_rhs(ctx, M, st->n_cap, st->t, st->mu, st->hist, &o);
       if (rc != DMFE_OK) return rc;
       st->n_rhs++;
     }
@@ -182,7 +182,7 @@ int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *acc
     // (PAPER.md:230); this evaluation is stage 1 of the next step.
     o.mu = st->mu + M;
     o.energy = st->energy ? st->energy + M : nullptr;
-    const int rc = dmfe_launch_rhs(ctx, M, st->t, st->mu, st->hist, &o);
+    const int rc = dmfe_launch_rhs(ctx, M, st->n_cap, st->t, st->mu, st->hist, &o);
     if (rc != DMFE_OK) return rc;
     st->n_rhs++;
     store_derivative_kernel<<<(L + 255) / 256, 256, 0, s>>>(L, M, st->hist, F);

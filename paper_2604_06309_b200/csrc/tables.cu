@@ -147,7 +147,7 @@ static int build_nu(const std::vector<double> &theta, int k, std::vector<double>
 //   start = clamp(l* - (s/2-1), 0, L-s)
 //   X(c)  = (L-1)(1+y)/2,  y = +-ln tan(B + c'(A-B))/gamma with c' = c (c <= 1/2) or the
 //           complement 1-c formed without cancellation (c > 1/2)   (G17)
-//   frac  = X - start
+//   frac  = X - start, stored packed with start in one 8-byte entry (dmfe_tab_encode)
 __device__ __forceinline__ int cell_of(const double *__restrict__ theta, int L, double c) {
   int lo = 0, hi = L - 1;  // theta[lo] <= c always holds (theta[0] = 0 <= c)
   while (lo < hi) {
@@ -171,7 +171,7 @@ __device__ __forceinline__ double index_coord(double c, double cbar, double A, d
 
 __global__ void pair_tables_kernel(int L, int s, double A, double B, double g,
                                    const double *__restrict__ theta, const double *__restrict__ omega,
-                                   int32_t *__restrict__ start, double *__restrict__ frac) {
+                                   uint64_t *__restrict__ tab) {
   const size_t plane = (size_t)L * (size_t)L;
   const int i = blockIdx.y;
   const double th_i = theta[i], om_i = omega[i];
@@ -196,8 +196,7 @@ __global__ void pair_tables_kernel(int L, int s, double A, double B, double g,
       int st = lstar - (s / 2 - 1);
       st = st < 0 ? 0 : (st > L - s ? L - s : st);
       const double X = index_coord(c[k], cb[k], A, B, g, L);
-      start[k * plane + e] = st;
-      frac[k * plane + e] = X - (double)st;
+      tab[k * plane + e] = dmfe_tab_encode(st, X - (double)st);
     }
   }
 }
@@ -217,8 +216,7 @@ int dmfe_build_tables(dmfe_ctx *ctx) {
   CUDA_TRY(ctx, cudaMalloc(&ctx->theta, vb));
   CUDA_TRY(ctx, cudaMalloc(&ctx->omega, vb));
   CUDA_TRY(ctx, cudaMalloc(&ctx->nu, vb));
-  CUDA_TRY(ctx, cudaMalloc(&ctx->start, 3 * plane * sizeof(int32_t)));
-  CUDA_TRY(ctx, cudaMalloc(&ctx->frac, 3 * plane * sizeof(double)));
+  CUDA_TRY(ctx, cudaMalloc(&ctx->tab, 3 * plane * sizeof(uint64_t)));
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->theta, theta.data(), vb, cudaMemcpyHostToDevice, ctx->stream));
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->omega, omega.data(), vb, cudaMemcpyHostToDevice, ctx->stream));
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->nu, nu.data(), vb, cudaMemcpyHostToDevice, ctx->stream));
@@ -227,7 +225,7 @@ int dmfe_build_tables(dmfe_ctx *ctx) {
   if (gx > 64) gx = 64;
   dim3 grid(gx, L);
   pair_tables_kernel<<<grid, nt, 0, ctx->stream>>>(L, s, ctx->A, ctx->B, ctx->gamma, ctx->theta,
-                                                    ctx->omega, ctx->start, ctx->frac);
+                                                    ctx->omega, ctx->tab);
   CUDA_TRY(ctx, cudaGetLastError());
   CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));  // host vectors go out of scope
   return DMFE_OK;
