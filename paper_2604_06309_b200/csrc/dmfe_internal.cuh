@@ -87,32 +87,33 @@ struct dmfe_ctx {
   } while (0)
 
 // Packed pair-table entry: bits 63..48 = stencil start (L <= 65535), bits 47..0 = the fractional
-// index coordinate u = X - start in fixed point: q = rint((u + 17) 2^44) - 2^48, i.e. the top 48
-// mantissa bits of the double u + 17 in [16, 32) (resolution 2^-44 = 5.7e-14 index units, far
-// below the ~4e-12 accuracy of X itself in fp64; -1 < u < 15 covers every stencil, s <= 10).
-// The decoded value is THE coordinate of the library: dmfe_get_tables returns it.
+// index coordinate u = X - start in fixed point, q = rint((u + 1) 2^44).  q is exactly the mantissa
+// field of the double x = 16 + (u + 1)/16 in [16, 17) (ulp 2^-48, top 16 bits 0x4030), so decoding
+// is one mask/or on the high word and one exact DFMA: u = 16 x - 257.  Resolution 2^-44 = 5.7e-14
+// index units (far below the ~4e-12 accuracy of X itself in fp64); -1 <= u < 15 covers every
+// stencil (s <= 10).  The decoded value is THE coordinate of the library: dmfe_get_tables returns it.
 #if defined(__CUDACC__)
 #define DMFE_HD __host__ __device__ __forceinline__
 #else
 #define DMFE_HD inline
 #endif
 DMFE_HD uint64_t dmfe_tab_encode(int32_t start, double frac) {
-  const double x = (frac + 17.0) * 17592186044416.0;  // 2^44: exact scaling
-  long long q = (long long)rint(x) - (16LL << 44);
+  const double x = (frac + 1.0) * 17592186044416.0;  // 2^44: exact scaling
+  long long q = (long long)rint(x);
   if (q < 0) q = 0;
   if (q > (1LL << 48) - 1) q = (1LL << 48) - 1;
   return ((uint64_t)(uint32_t)start << 48) | (uint64_t)q;
 }
 DMFE_HD void dmfe_tab_decode(uint64_t e, int32_t *start, double *frac) {
   *start = (int32_t)(e >> 48);
-  const uint64_t bits = 0x4030000000000000ULL | ((e & 0xFFFFFFFFFFFFULL) << 4);
+  const uint64_t bits = 0x4030000000000000ULL | (e & 0xFFFFFFFFFFFFULL);
   double x;
 #if defined(__CUDA_ARCH__)
   x = __longlong_as_double((long long)bits);
 #else
   memcpy(&x, &bits, sizeof(x));
 #endif
-  *frac = x - 17.0;
+  *frac = x * 16.0 - 257.0;  // exact: x has at most 48 significant fraction bits below 2^4
 }
 
 // tables.cu

@@ -24,6 +24,9 @@
 namespace {
 
 constexpr int RHS_THREADS = 256;
+#ifndef DMFE_MINB
+#define DMFE_MINB 3
+#endif
 constexpr int PREP_THREADS = 1024;
 
 struct RhsArgs {
@@ -55,6 +58,26 @@ __device__ __forceinline__ uint64_t ld_stream(const uint64_t *p) {
 __device__ __forceinline__ double horner(const double *c, int deg, double q) {
   double acc = c[deg];
   for (int k = deg - 1; k >= 0; --k) acc = fma(acc, q, c[k]);
+  return acc;
+}
+
+// f'(q) and f''(q) with the polynomial degree fixed at compile time (PD = degree of f; the
+// coefficient arrays are zero beyond p_max, so a model with p_max < PD evaluates exactly the same
+// value); PD = 0 selects the run-time loop.
+template <int PD>
+__device__ __forceinline__ double f1(const ModelCoef &mc, double q) {
+  if (PD == 0) return horner(mc.c1, mc.pmax - 1, q);
+  double acc = mc.c1[PD - 1];
+#pragma unroll
+  for (int k = PD - 2; k >= 0; --k) acc = fma(acc, q, mc.c1[k]);
+  return acc;
+}
+template <int PD>
+__device__ __forceinline__ double f2(const ModelCoef &mc, double q) {
+  if (PD == 0) return horner(mc.c2, mc.pmax - 2, q);
+  double acc = mc.c2[PD - 2];
+#pragma unroll
+  for (int k = PD - 3; k >= 0; --k) acc = fma(acc, q, mc.c2[k]);
   return acc;
 }
 
@@ -170,15 +193,14 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int S>
-__global__ void __launch_bounds__(RHS_THREADS, 3) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
+template <int S, int PD>
+__global__ void __launch_bounds__(RHS_THREADS, DMFE_MINB) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
   const int L = a.L, M = a.M;
   const int i = blockIdx.x;
   const size_t plane = (size_t)L * (size_t)L;
   const uint64_t *tab1 = a.tab + (size_t)i * (size_t)L, *tab2 = tab1 + plane, *tab3 = tab2 + plane;
   const double th_i = a.theta[i], om_i = a.omega[i];
   const double tM = a.t[M];
-  const int d1 = mc.pmax - 1, d2 = mc.pmax - 2;
 
   // type-1: one row search per target, tau = theta_i t  (Eq.(19)); blo[i] is exactly that row
   const double tau1 = __dmul_rn(th_i, tM);
@@ -198,14 +220,26 @@ __global__ void __launch_bounds__(RHS_THREADS, 3) history_integrals_kernel(RhsAr
   __shared__ double red[RHS_THREADS / 32][8];
   __shared__ double b1c_first;
 
+  // the table stream of the next iteration is fetched one iteration ahead (its DRAM latency is
+  // the head of a chain of dependent gathers)
+  uint64_t e1 = 0, e2 = 0, e3 = 0;
+  if (threadIdx.x < L) {
+    e1 = ld_stream(tab1 + threadIdx.x);
+    e2 = ld_stream(tab2 + threadIdx.x);
+    e3 = ld_stream(tab3 + threadIdx.x);
+  }
   for (int j = threadIdx.x; j < L; j += RHS_THREADS) {
-    const uint64_t e1 = ld_stream(tab1 + j), e2 = ld_stream(tab2 + j), e3 = ld_stream(tab3 + j);
     const double nj = a.nu[j];
     int a1, a2, a3;
     double u1, u2, u3;
     dmfe_tab_decode(e1, &a1, &u1);
     dmfe_tab_decode(e2, &a2, &u2);
     dmfe_tab_decode(e3, &a3, &u3);
+    if (j + RHS_THREADS < L) {
+      e1 = ld_stream(tab1 + j + RHS_THREADS);
+      e2 = ld_stream(tab2 + j + RHS_THREADS);
+      e3 = ld_stream(tab3 + j + RHS_THREADS);
+    }
     double w[S];
     // ---- A factors at phi1 (Eq.(18)) and the type-1 lookup (Eq.(19)): sums S1, S3, S5, S6 ----
     {
@@ -223,10 +257,10 @@ __global__ void __launch_bounds__(RHS_THREADS, 3) history_integrals_kernel(RhsAr
       const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
       const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
       if (j == 0) b1c_first = B1C;
-      acc[0] = fma(nj * (horner(mc.c2, d2, C1) * R1), B1C, acc[0]);   // S1: K(t,s) C(t',s)
-      acc[2] = fma(nj * horner(mc.c1, d1, C1), B1R, acc[2]);          // S3: D(t,s) R(t',s)
-      acc[4] = fma(nj * (horner(mc.c2, d2, B1C) * B1R), C1, acc[4]);  // S5: K(t',s) C(t,s)
-      acc[5] = fma(nj * horner(mc.c1, d1, B1C), R1, acc[5]);          // S6: D(t',s) R(t,s)
+      acc[0] = fma(nj * (f2<PD>(mc, C1) * R1), B1C, acc[0]);   // S1: K(t,s) C(t',s)
+      acc[2] = fma(nj * f1<PD>(mc, C1), B1R, acc[2]);          // S3: D(t,s) R(t',s)
+      acc[4] = fma(nj * (f2<PD>(mc, B1C) * B1R), C1, acc[4]);  // S5: K(t',s) C(t,s)
+      acc[5] = fma(nj * f1<PD>(mc, B1C), R1, acc[5]);          // S6: D(t',s) R(t,s)
     }
     // ---- A factors at phi2 (Eq.(18)) ----
     double C2 = 0.0, R2 = 0.0;
@@ -271,11 +305,11 @@ __global__ void __launch_bounds__(RHS_THREADS, 3) history_integrals_kernel(RhsAr
     const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
     // ---- kernel functions (Eq.(10)-(11)) and the type-2 terms (Eq.(21)) ----
     const double nR2 = nj * R2;
-    const double K2 = horner(mc.c2, d2, C2) * nR2;
+    const double K2 = f2<PD>(mc, C2) * nR2;
     acc[1] = fma(K2, B2C, acc[1]);                                   // S2: K(t,s) C(s,t')
     acc[3] = fma(K2, B2R, acc[3]);                                   // S4: K(t,s) R(s,t')
-    acc[6] = fma(horner(mc.c1, d1, B2C), nR2, acc[6]);               // S7: D(s,t') R(t,s)
-    acc[7] = fma(nR2, horner(mc.c2, d2, B2C) * B2R, acc[7]);         // S8: R(t,s) K(s,t')
+    acc[6] = fma(f1<PD>(mc, B2C), nR2, acc[6]);               // S7: D(s,t') R(t,s)
+    acc[7] = fma(nR2, f2<PD>(mc, B2C) * B2R, acc[7]);         // S8: R(t,s) K(s,t')
   }
   // ---- reduction over j: shuffle within the warp, fixed order across warps ----
 #pragma unroll
@@ -315,8 +349,8 @@ __global__ void __launch_bounds__(RHS_THREADS, 3) history_integrals_kernel(RhsAr
     mu_p += wgt * mv;
   }
   const double2 ci = a.cur[i], c0 = a.cur[0];
-  const double fc = mc.beta0 * horner(mc.c1, d1, c0.x) * b1c_first;
-  const double fc2 = mc.beta0 * horner(mc.c1, d1, b1c_first) * c0.x;
+  const double fc = mc.beta0 * f1<PD>(mc, c0.x) * b1c_first;
+  const double fc2 = mc.beta0 * f1<PD>(mc, b1c_first) * c0.x;
   const double d1C = -mu * ci.x + tM * (th_i * Sd[0] + om_i * Sd[1] + th_i * Sd[2]) + fc;
   const double d1R = -mu * ci.y + tM * (om_i * Sd[3]);
   const double d2C = -mu_p * ci.x + tM * (th_i * Sd[4] + th_i * Sd[5] + om_i * Sd[6]) + 2.0 * mc.T * ci.y + fc2;
@@ -379,14 +413,30 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
     }
     CUDA_TRY(ctx, cudaEventRecord(ctx->ev[2 * ctx->ev_n], ctx->stream));
   }
+  // the polynomial degree of f is a compile-time constant for p_max <= 4 (the paper's models
+  // p = 2, 3, 2+4, 3+4, 2+3+4); larger p_max (3+9) takes the run-time Horner loop
+  const int pd = ctx->model.pmax <= 3 ? 3 : (ctx->model.pmax == 4 ? 4 : 0);
+#define DMFE_LAUNCH(S_, PD_) \
+  history_integrals_kernel<S_, PD_><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model)
+#define DMFE_LAUNCH_S(S_)        \
+  do {                           \
+    if (pd == 3)                 \
+      DMFE_LAUNCH(S_, 3);        \
+    else if (pd == 4)            \
+      DMFE_LAUNCH(S_, 4);        \
+    else                         \
+      DMFE_LAUNCH(S_, 0);        \
+  } while (0)
   switch (ctx->p.stencil) {
-    case 2: history_integrals_kernel<2><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
-    case 4: history_integrals_kernel<4><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
-    case 6: history_integrals_kernel<6><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
-    case 8: history_integrals_kernel<8><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
-    case 10: history_integrals_kernel<10><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model); break;
+    case 2: DMFE_LAUNCH_S(2); break;
+    case 4: DMFE_LAUNCH_S(4); break;
+    case 6: DMFE_LAUNCH_S(6); break;
+    case 8: DMFE_LAUNCH_S(8); break;
+    case 10: DMFE_LAUNCH_S(10); break;
     default: return DMFE_EINVAL;
   }
+#undef DMFE_LAUNCH_S
+#undef DMFE_LAUNCH
   if (timed) {
     CUDA_TRY(ctx, cudaEventRecord(ctx->ev[2 * ctx->ev_n + 1], ctx->stream));
     ctx->ev_n++;
