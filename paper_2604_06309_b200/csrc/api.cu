@@ -29,6 +29,7 @@ static void free_all(dmfe_ctx *c) {
   cudaFree(c->theta);
   cudaFree(c->omega);
   cudaFree(c->nu);
+  cudaFree(c->thnu);
   cudaFree(c->tab);
   cudaFree(c->blo);
   cudaFree(c->rowtab);
@@ -75,6 +76,13 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
   double f2_1 = 0.0;  // f''(1) for the step cap of Eq.(24)
   for (int k = 0; k <= p.p_max; ++k) f2_1 += m.c2[k];
   c->h_stab = (f2_1 > 0.0) ? 13.9 / (4.0 * sqrt(f2_1)) : INFINITY;
+  {
+    int dev = 0, v = 0;
+    cudaGetDevice(&dev);
+    c->sm_count = (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) ? v : 148;
+    c->smem_max = (cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) == cudaSuccess && v > 0)
+                      ? v - 2048 : 46 * 1024;
+  }
   int rc = dmfe_build_tables(c);
   const int L = p.L;
   if (rc == DMFE_OK) {

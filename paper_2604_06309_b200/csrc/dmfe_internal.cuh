@@ -45,15 +45,18 @@ struct dmfe_ctx {
   ModelCoef model;
   cudaStream_t stream;
   int cuda_err;
+  int sm_count;  // SMs of the device the context was created on
+  int smem_max;  // opt-in dynamic shared memory per CTA, minus the kernels' static use
   double gamma, A, B;  // gamma = -W_{-1}(-1/t_max); A = atan(e^gamma), B = atan(e^-gamma)
   double h_stab;       // 13.9 / (4 sqrt(f''(1)))  (Eq.(24))
   // ---- tables (device) ----
   double *theta, *omega, *nu;  // [L]
+  double2 *thnu;               // [L] {theta_j, nu_j}
   uint64_t *tab;               // [3][L][L] packed {stencil start : 16 | fractional coordinate : 48}
   // ---- O(L) scratch (device) ----
   double2 *cur;     // [L] {C, R} of the current row, packed for 16-byte gathers
   int32_t *blo;     // [L] per-call row bracket table: blo[c] = n(theta_c t_M)
-  double2 *rowtab;  // [rowtab_cap] per-call {t_n, t_{n+1} - t_n}
+  double2 *rowtab;  // [rowtab_cap] per-call {t_n, 1 / (t_{n+1} - t_n)}
   int32_t rowtab_cap;
   double *scal;     // [SC_COUNT]
   int32_t *iscal;   // [IS_COUNT]

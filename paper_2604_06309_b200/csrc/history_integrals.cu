@@ -9,29 +9,38 @@
 // and the O(L) parts: mu(t) Eq.(13), E(t) Eq.(14), the right-hand sides of Eq.(1) and of the
 // second-argument equations (readings G1, G9, G10 in DESIGN.md), the ray derivative of Eq.(22).
 //
-// Mapping: one CTA per target i, lanes <-> adjacent nodes j (type-1 rows and the pair tables are
-// read coalesced; the type-2 cells of adjacent lanes are neighbours in the packed history).
-// Every history cell {C,dC,R,dR} is one 256-bit load.  fp64 throughout; no tensor cores: every
-// "matrix" here is a gather.
+// Mapping: persistent kernel, one CTA per SM.  The CTA's warps form groups of G warps; a group
+// evaluates one target i at a time, lanes <-> adjacent nodes j (type-1 rows and the pair tables
+// are read coalesced; the type-2 cells of adjacent lanes are neighbours in the packed history);
+// the groups of one CTA take adjacent targets.  Every history cell {C,dC,R,dR} is one 256-bit
+// load.  The per-call O(L + M) tables (current row, row table, bracket table) are copied into
+// shared memory once per CTA when they fit.  fp64 throughout; no tensor cores: every "matrix"
+// here is a gather.
 //
 // Launch 1 (prepare_kernel, O(L + M)): packs row M into {C,R} pairs, reduces mu and E, builds the
-// per-call row table {t_n, t_{n+1}-t_n} and the row bracket table blo[c] = n(theta_c t_M).
+// per-call row table {t_n, 1/(t_{n+1}-t_n)} and the row bracket table blo[c] = n(theta_c t_M).
 // Launch 2 (history_integrals_kernel): the L^2 pairs.  The row search of a pair is
-// a bisection inside the bracket [blo[a], blo[b]] given by the grid cells a <= phi2 < b that the
-// phi2 stencil start already identifies -- same predicate and same result as a full bisection.
+// a bisection inside the bracket [blo[l*], blo[l*+1]] of the grid cell theta_l* <= phi2 < theta_l*+1
+// that the phi2 stencil start already identifies -- same predicate and same result as a full
+// bisection.  The loop over j is software-pipelined: while pair p is evaluated, the table entries
+// of pair p+2 are in flight and the index stage of pair p+1 (bracket, bisection) has run.
 #include "dmfe_internal.cuh"
 
 namespace {
 
-constexpr int RHS_THREADS = 256;
-#ifndef DMFE_MINB
-#define DMFE_MINB 3
+#ifndef DMFE_THREADS
+#define DMFE_THREADS 512
 #endif
+#ifndef DMFE_PRELOAD
+#define DMFE_PRELOAD 0  // 1: all type-2 cell loads of a pair issued before the index stage of the next
+#endif
+constexpr int RHS_THREADS = DMFE_THREADS;
 constexpr int PREP_THREADS = 1024;
 
 struct RhsArgs {
   int32_t L, M;
-  const double *theta, *omega, *nu;
+  const double *theta, *omega;
+  const double2 *thnu;
   const uint64_t *tab;
   const double *t, *mu_hist;
   const double4 *hist;
@@ -39,6 +48,7 @@ struct RhsArgs {
   const double2 *rowtab;
   const int32_t *blo;
   const double *scal;  // SC_MU, SC_E written by prepare_kernel
+  int32_t G;           // warps per target group
   dmfe_rhs_out out;
 };
 
@@ -52,7 +62,9 @@ __device__ __forceinline__ double4 ld_cell(const double4 *p) {
 
 // streamed once per call: keep it out of L1 and first in line for L2 eviction
 __device__ __forceinline__ uint64_t ld_stream(const uint64_t *p) {
-  return (uint64_t)__ldcs((const unsigned long long *)p);
+  unsigned long long v;
+  asm volatile("ld.global.nc.L1::no_allocate.b64 %0, [%1];" : "=l"(v) : "l"(p));
+  return (uint64_t)v;
 }
 
 __device__ __forceinline__ double horner(const double *c, int deg, double q) {
@@ -117,30 +129,33 @@ __device__ __forceinline__ int row_search(const double *__restrict__ t, int lo, 
 }
 
 // weights of the local interpolant in t between rows n and n+1 (PAPER.md:260 cubic Hermite);
-// quadratic (value, slope, value) when the upper row is the current row M (reading G12).
-//   h00 = 2u^3-3u^2+1, h10 = u(u-1)^2 D, h01 = 1-h00, h11 = u^2(u-1) D;  top: 1-u^2, u(1-u) D, u^2, 0
-__device__ __forceinline__ void t_weights(double tn, double D, double tau, bool top, double (&h)[4]) {
-  const double u = (tau - tn) / D;
+// quadratic (value, slope, value) when the upper row is the current row M (reading G12).  With
+// d = tau - t_n, u = d/D, v = u - 1:
+//   h00 = 2u^3-3u^2+1, h10 = u v^2 D = d v^2, h01 = 1-h00, h11 = u^2 v D = d u v;  top: 1-u^2, -d v, u^2, 0
+// rD = 1/D comes from the per-call row table, so a pair costs no division.
+__device__ __forceinline__ void t_weights(double tn, double rD, double tau, bool top, double (&h)[4]) {
+  const double d = tau - tn;
+  const double u = d * rD;
   const double v = u - 1.0;
   const double u2 = u * u;
-  const double uvD = u * v * D;
+  const double dv = d * v;
   if (top) {
     h[0] = 1.0 - u2;
-    h[1] = -uvD;
+    h[1] = -dv;
     h[2] = u2;
     h[3] = 0.0;
   } else {
     h[0] = fma(u2, fma(2.0, u, -3.0), 1.0);
-    h[1] = uvD * v;
+    h[1] = dv * v;
     h[2] = 1.0 - h[0];
-    h[3] = uvD * u;
+    h[3] = dv * u;
   }
 }
 
 // ---------------------------------------------------------------------------------------------
 // O(L + M) pre-pass.  Block 0: pack row M into {C,R} pairs and reduce mu(t) (Eq.(13)) and E(t)
 // (Eq.(14)).  Blocks >= 1 (or block 0 too when launched alone): the per-call row table
-// rowtab[n] = {t_n, t_{n+1} - t_n}, n < M, and the bracket table blo[c] = n(fl(theta_c t_M)):
+// rowtab[n] = {t_n, 1/(t_{n+1} - t_n)}, n < M, and the bracket table blo[c] = n(fl(theta_c t_M)):
 // for theta_a <= phi < theta_b rounding is monotone, so n(fl(phi t_M)) lies in [blo[a], blo[b]].
 __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, ModelCoef mc,
                                                                const double *__restrict__ theta,
@@ -156,7 +171,7 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
     for (int e = b * PREP_THREADS + threadIdx.x; e < M + L; e += nb * PREP_THREADS) {
       if (e < M) {
         const double tn = t[e];
-        rowtab[e] = make_double2(tn, t[e + 1] - tn);
+        rowtab[e] = make_double2(tn, 1.0 / (t[e + 1] - tn));
       } else {
         const int c = e - M;
         blo[c] = row_search(t, 0, M - 1, __dmul_rn(theta[c], tM));
@@ -193,179 +208,292 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int S, int PD>
-__global__ void __launch_bounds__(RHS_THREADS, DMFE_MINB) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
+// Small per-call tables (current row, row table, bracket table) live in shared memory when they
+// fit (SM = true): the gathers into them are the head of every pair's dependent load chain, and
+// the history cells streaming through L1 (1 KB per warp-wide load) would otherwise evict them
+// once per iteration.  SM = false reads the same arrays from global memory.
+template <bool SM, class T>
+__device__ __forceinline__ T ld_tab(const T *p) {
+  if (SM) return *p;
+  return __ldg(p);
+}
+
+// n = max{ n in [lo, hi] : rowtab[n].x <= tau }; requires t[lo] <= tau.
+template <bool SM>
+__device__ __forceinline__ int row_search_tab(const double2 *rowtab, int lo, int hi, double tau) {
+  while (lo < hi) {
+    const int mid = lo + ((hi - lo + 1) >> 1);
+    if (ld_tab<SM>(&rowtab[mid].x) <= tau)
+      lo = mid;
+    else
+      hi = mid - 1;
+  }
+  return lo;
+}
+
+// Index stage of one pair (the integer half of Eq.(20)): tau2 = fl(phi2 t_M) and its
+// row n2, found by bisection inside the bracket of the grid cell of phi2.  l* = max{l : theta_l <=
+// phi2} equals a2 + S/2 - 1 unless the stencil start was clamped, in which case l* lies in
+// [0, S/2-1] (a2 = 0) or [L-S/2-1, L-1] (a2 = L-S).  n2 <= M-1, so the search runs on rowtab[0..M-1].
+template <int S, bool SM>
+__device__ __forceinline__ int index_stage(const double2 *rowtab, const int32_t *blo, const double4 *hist, int L,
+                                           double th_i, double om_i, double tM, double th_j, int a2, int a3,
+                                           double *tau2_out) {
+  const double phi2 = __dadd_rn(th_i, __dmul_rn(om_i, th_j));
+  const double tau2 = __dmul_rn(phi2, tM);
+  int clo = a2 + (S / 2 - 1), chi = clo + 1;
+  if (a2 == 0) clo = 0, chi = S / 2;
+  if (a2 == L - S) clo = (a2 == 0) ? 0 : L - S / 2 - 1, chi = L - 1;
+  const int n2 = row_search_tab<SM>(rowtab, ld_tab<SM>(blo + clo), ld_tab<SM>(blo + chi), tau2);
+  *tau2_out = tau2;
+  return n2;
+}
+
+__device__ __forceinline__ void group_barrier(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// Persistent kernel: one CTA per SM; the CTA's warps form groups of G warps, a group evaluates one
+// target i at a time (lanes <-> adjacent nodes j), groups of one CTA take adjacent targets.
+template <int S, int PD, bool SM>
+__global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
+  extern __shared__ double4 smem_dyn[];
   const int L = a.L, M = a.M;
-  const int i = blockIdx.x;
+  const double2 *cur = a.cur;
+  const double2 *rowtab = a.rowtab;
+  const int32_t *blo = a.blo;
+  if (SM) {
+    double2 *s_cur = reinterpret_cast<double2 *>(smem_dyn);
+    double2 *s_row = s_cur + L;
+    int32_t *s_blo = reinterpret_cast<int32_t *>(s_row + M);
+    for (int k = threadIdx.x; k < L; k += RHS_THREADS) s_cur[k] = a.cur[k], s_blo[k] = a.blo[k];
+    for (int k = threadIdx.x; k < M; k += RHS_THREADS) s_row[k] = a.rowtab[k];
+    __syncthreads();
+    cur = s_cur, rowtab = s_row, blo = s_blo;
+  }
+  __shared__ double red[2][RHS_THREADS / 32][8];
+
+  const int G = a.G;                 // warps per group (power of two, <= RHS_THREADS/32)
+  const int TG = 32 * G;             // threads per group = stride of j
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int group = warp / G, wg = warp % G;
+  const int ngroups = (RHS_THREADS / 32) / G;
+  const int tig = wg * 32 + lane;    // thread index inside the group
   const size_t plane = (size_t)L * (size_t)L;
-  const uint64_t *tab1 = a.tab + (size_t)i * (size_t)L, *tab2 = tab1 + plane, *tab3 = tab2 + plane;
-  const double th_i = a.theta[i], om_i = a.omega[i];
   const double tM = a.t[M];
+  int parity = 0;
 
-  // type-1: one row search per target, tau = theta_i t  (Eq.(19)); blo[i] is exactly that row
-  const double tau1 = __dmul_rn(th_i, tM);
-  const int n1 = a.blo[i];
-  const bool top1 = (n1 + 1 == M);
-  double h1[4];
-  {
-    const double2 rt = a.rowtab[n1];
-    t_weights(rt.x, rt.y, tau1, top1, h1);
-  }
-  const double4 *row1lo = a.hist + (size_t)n1 * (size_t)L;
-  const double4 *row1hi = row1lo + L;
-
-  double acc[8];
-#pragma unroll
-  for (int k = 0; k < 8; ++k) acc[k] = 0.0;
-  __shared__ double red[RHS_THREADS / 32][8];
-  __shared__ double b1c_first;
-
-  // the table stream of the next iteration is fetched one iteration ahead (its DRAM latency is
-  // the head of a chain of dependent gathers)
-  uint64_t e1 = 0, e2 = 0, e3 = 0;
-  if (threadIdx.x < L) {
-    e1 = ld_stream(tab1 + threadIdx.x);
-    e2 = ld_stream(tab2 + threadIdx.x);
-    e3 = ld_stream(tab3 + threadIdx.x);
-  }
-  for (int j = threadIdx.x; j < L; j += RHS_THREADS) {
-    const double nj = a.nu[j];
-    int a1, a2, a3;
-    double u1, u2, u3;
-    dmfe_tab_decode(e1, &a1, &u1);
-    dmfe_tab_decode(e2, &a2, &u2);
-    dmfe_tab_decode(e3, &a3, &u3);
-    if (j + RHS_THREADS < L) {
-      e1 = ld_stream(tab1 + j + RHS_THREADS);
-      e2 = ld_stream(tab2 + j + RHS_THREADS);
-      e3 = ld_stream(tab3 + j + RHS_THREADS);
-    }
-    double w[S];
-    // ---- A factors at phi1 (Eq.(18)) and the type-1 lookup (Eq.(19)): sums S1, S3, S5, S6 ----
+  for (int i = blockIdx.x * ngroups + group; i < L; i += gridDim.x * ngroups, parity ^= 1) {
+    const uint64_t *tab1 = a.tab + (size_t)i * (size_t)L, *tab2 = tab1 + plane, *tab3 = tab2 + plane;
+    const double th_i = a.theta[i], om_i = a.omega[i];
+    // type-1: one row search per target, tau = theta_i t  (Eq.(19)); blo[i] is exactly that row
+    const double tau1 = __dmul_rn(th_i, tM);
+    const int n1 = ld_tab<SM>(blo + i);
+    const bool top1 = (n1 + 1 == M);
+    double h1[4];
     {
-      double C1 = 0.0, R1 = 0.0;
-      lagrange_weights<S>(u1, w);
+      const double2 rt = ld_tab<SM>(rowtab + n1);
+      t_weights(rt.x, rt.y, tau1, top1, h1);
+    }
+    const double4 *row1lo = a.hist + (size_t)n1 * (size_t)L;
+    const double4 *row1hi = row1lo + L;
+
+    double acc[8];
 #pragma unroll
-      for (int l = 0; l < S; ++l) {
-        const double2 v = __ldg(a.cur + a1 + l);
-        C1 = fma(w[l], v.x, C1);
-        R1 = fma(w[l], v.y, R1);
+    for (int k = 0; k < 8; ++k) acc[k] = 0.0;
+    double b1c_first = 0.0;
+
+    // ---- software pipeline over this thread's pairs p = j, j + TG, j + 2 TG, ... ----
+    //   eA*: table entries of the pair being evaluated; n2A / tau2A: its row and time
+    //   eB*, thB: table entries and theta_j of the next pair; eC*, thC: in flight for the one after
+    uint64_t eA1 = 0, eA2 = 0, eA3 = 0, eB1 = 0, eB2 = 0, eB3 = 0;
+    double2 tnA = make_double2(0.0, 0.0), tnB = tnA;
+    int n2A = 0;
+    double tau2A = 0.0;
+    int j = tig;
+    if (j < L) {
+      eA1 = ld_stream(tab1 + j);
+      eA2 = ld_stream(tab2 + j);
+      eA3 = ld_stream(tab3 + j);
+      tnA = __ldg(a.thnu + j);
+    }
+    if (j + TG < L) {
+      eB1 = ld_stream(tab1 + j + TG);
+      eB2 = ld_stream(tab2 + j + TG);
+      eB3 = ld_stream(tab3 + j + TG);
+      tnB = __ldg(a.thnu + j + TG);
+    }
+    if (j < L)
+      n2A = index_stage<S, SM>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnA.x, (int)(eA2 >> 48), (int)(eA3 >> 48),
+                               &tau2A);
+    for (; j < L; j += TG) {
+      uint64_t eC1 = 0, eC2 = 0, eC3 = 0;
+      double2 tnC = make_double2(0.0, 0.0);
+      if (j + 2 * TG < L) {
+        eC1 = ld_stream(tab1 + j + 2 * TG);
+        eC2 = ld_stream(tab2 + j + 2 * TG);
+        eC3 = ld_stream(tab3 + j + 2 * TG);
+        tnC = __ldg(a.thnu + j + 2 * TG);
       }
+      // type-1 cells and type-2 cells of this pair: issue all ten 32-byte loads up front
       const double4 lo = ld_cell(row1lo + j);
       double4 hi = ld_cell(row1hi + j);
-      if (top1) hi.y = 0.0, hi.w = 0.0;
-      const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
-      const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
-      if (j == 0) b1c_first = B1C;
-      acc[0] = fma(nj * (f2<PD>(mc, C1) * R1), B1C, acc[0]);   // S1: K(t,s) C(t',s)
-      acc[2] = fma(nj * f1<PD>(mc, C1), B1R, acc[2]);          // S3: D(t,s) R(t',s)
-      acc[4] = fma(nj * (f2<PD>(mc, B1C) * B1R), C1, acc[4]);  // S5: K(t',s) C(t,s)
-      acc[5] = fma(nj * f1<PD>(mc, B1C), R1, acc[5]);          // S6: D(t',s) R(t,s)
-    }
-    // ---- A factors at phi2 (Eq.(18)) ----
-    double C2 = 0.0, R2 = 0.0;
-    lagrange_weights<S>(u2, w);
+      const int n2 = n2A;
+      const int a3 = (int)(eA3 >> 48);
+      const double4 *p2 = a.hist + (size_t)n2 * (size_t)L + a3;
+#if DMFE_PRELOAD
+      double4 x[S], y[S];
 #pragma unroll
-    for (int l = 0; l < S; ++l) {
-      const double2 v = __ldg(a.cur + a2 + l);
-      C2 = fma(w[l], v.x, C2);
-      R2 = fma(w[l], v.y, R2);
-    }
-    // ---- type-2 lookup (Eq.(20)): row search in the bracket of the phi2 grid cells ----
-    const double phi2 = __dadd_rn(th_i, __dmul_rn(om_i, a.theta[j]));
-    const double tau2 = __dmul_rn(phi2, tM);
-    const int chi = (a2 == L - S) ? L - 1 : a2 + S / 2;
-    const int n2 = row_search(a.t, __ldg(a.blo + a2), __ldg(a.blo + chi), tau2);
-    if (a.out.rows2) a.out.rows2[(size_t)i * (size_t)L + (size_t)j] = n2;
-    const bool top2 = (n2 + 1 == M);
-    double h2[4];
-    {
-      const double2 rt = __ldg(a.rowtab + n2);
-      t_weights(rt.x, rt.y, tau2, top2, h2);
-    }
-    // theta-stencil first, then t
-    lagrange_weights<S>(u3, w);
-    const double4 *p2 = a.hist + (size_t)n2 * (size_t)L + a3;
-    double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
-#pragma unroll
-    for (int l = 0; l < S; ++l) {
-      const double4 x = ld_cell(p2 + l);
-      const double4 y = ld_cell(p2 + L + l);
-      cl = fma(w[l], x.x, cl);
-      dcl = fma(w[l], x.y, dcl);
-      rl = fma(w[l], x.z, rl);
-      drl = fma(w[l], x.w, drl);
-      cu = fma(w[l], y.x, cu);
-      dcu = fma(w[l], y.y, dcu);
-      ru = fma(w[l], y.z, ru);
-      dru = fma(w[l], y.w, dru);
-    }
-    if (top2) dcu = 0.0, dru = 0.0;
-    const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
-    const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
-    // ---- kernel functions (Eq.(10)-(11)) and the type-2 terms (Eq.(21)) ----
-    const double nR2 = nj * R2;
-    const double K2 = f2<PD>(mc, C2) * nR2;
-    acc[1] = fma(K2, B2C, acc[1]);                                   // S2: K(t,s) C(s,t')
-    acc[3] = fma(K2, B2R, acc[3]);                                   // S4: K(t,s) R(s,t')
-    acc[6] = fma(f1<PD>(mc, B2C), nR2, acc[6]);               // S7: D(s,t') R(t,s)
-    acc[7] = fma(nR2, f2<PD>(mc, B2C) * B2R, acc[7]);         // S8: R(t,s) K(s,t')
-  }
-  // ---- reduction over j: shuffle within the warp, fixed order across warps ----
-#pragma unroll
-  for (int k = 0; k < 8; ++k)
-    for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
-  const int wid = threadIdx.x >> 5;
-  if ((threadIdx.x & 31) == 0) {
-#pragma unroll
-    for (int k = 0; k < 8; ++k) red[wid][k] = acc[k];
-  }
-  __syncthreads();
-  if (threadIdx.x != 0) return;
+      for (int l = 0; l < S; ++l) {
+        x[l] = ld_cell(p2 + l);
+        y[l] = ld_cell(p2 + L + l);
+      }
+#endif
+      // index stage of the next pair (shared-memory chain) while those loads are in flight
+      int n2B = 0;
+      double tau2B = 0.0;
+      if (j + TG < L)
+        n2B = index_stage<S, SM>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnB.x, (int)(eB2 >> 48),
+                                 (int)(eB3 >> 48), &tau2B);
 
-  double Sd[8];
+      const double nj = tnA.y;
+      int a1, a2, a3d;
+      double u1, u2, u3;
+      dmfe_tab_decode(eA1, &a1, &u1);
+      dmfe_tab_decode(eA2, &a2, &u2);
+      dmfe_tab_decode(eA3, &a3d, &u3);
+      double w[S];
+      // ---- A factors at phi1 (Eq.(18)) and the type-1 lookup (Eq.(19)): sums S1, S3, S5, S6 ----
+      {
+        double C1 = 0.0, R1 = 0.0;
+        lagrange_weights<S>(u1, w);
 #pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    double s = 0.0;
-    for (int w = 0; w < RHS_THREADS / 32; ++w) s += red[w][k];
-    Sd[k] = s;
-    if (a.out.sums) a.out.sums[(size_t)k * L + i] = s;
-  }
-  if (a.out.rows1) a.out.rows1[i] = n1;
+        for (int l = 0; l < S; ++l) {
+          const double2 v = ld_tab<SM>(cur + a1 + l);
+          C1 = fma(w[l], v.x, C1);
+          R1 = fma(w[l], v.y, R1);
+        }
+        if (top1) hi.y = 0.0, hi.w = 0.0;
+        const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
+        const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
+        if (j == 0) b1c_first = B1C;
+        acc[0] = fma(nj * (f2<PD>(mc, C1) * R1), B1C, acc[0]);   // S1: K(t,s) C(t',s)
+        acc[2] = fma(nj * f1<PD>(mc, C1), B1R, acc[2]);          // S3: D(t,s) R(t',s)
+        acc[4] = fma(nj * (f2<PD>(mc, B1C) * B1R), C1, acc[4]);  // S5: K(t',s) C(t,s)
+        acc[5] = fma(nj * f1<PD>(mc, B1C), R1, acc[5]);          // S6: D(t',s) R(t,s)
+      }
+      // ---- A factors at phi2 (Eq.(18)) ----
+      double C2 = 0.0, R2 = 0.0;
+      lagrange_weights<S>(u2, w);
+#pragma unroll
+      for (int l = 0; l < S; ++l) {
+        const double2 v = ld_tab<SM>(cur + a2 + l);
+        C2 = fma(w[l], v.x, C2);
+        R2 = fma(w[l], v.y, R2);
+      }
+      // ---- type-2 lookup (Eq.(20)) in the rows n2, n2+1 found by the index stage ----
+      if (a.out.rows2) a.out.rows2[(size_t)i * (size_t)L + (size_t)j] = n2;
+      const bool top2 = (n2 + 1 == M);
+      double h2[4];
+      {
+        const double2 rt = ld_tab<SM>(rowtab + n2);
+        t_weights(rt.x, rt.y, tau2A, top2, h2);
+      }
+      // theta-stencil first, then t
+      lagrange_weights<S>(u3, w);
+      double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
+#pragma unroll
+      for (int l = 0; l < S; ++l) {
+#if DMFE_PRELOAD
+        const double4 xl = x[l], yl = y[l];
+#else
+        const double4 xl = ld_cell(p2 + l), yl = ld_cell(p2 + L + l);
+#endif
+        cl = fma(w[l], xl.x, cl);
+        dcl = fma(w[l], xl.y, dcl);
+        rl = fma(w[l], xl.z, rl);
+        drl = fma(w[l], xl.w, drl);
+        cu = fma(w[l], yl.x, cu);
+        dcu = fma(w[l], yl.y, dcu);
+        ru = fma(w[l], yl.z, ru);
+        dru = fma(w[l], yl.w, dru);
+      }
+      if (top2) dcu = 0.0, dru = 0.0;
+      const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
+      const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
+      // ---- kernel functions (Eq.(10)-(11)) and the type-2 terms (Eq.(21)) ----
+      const double nR2 = nj * R2;
+      const double K2 = f2<PD>(mc, C2) * nR2;
+      acc[1] = fma(K2, B2C, acc[1]);                            // S2: K(t,s) C(s,t')
+      acc[3] = fma(K2, B2R, acc[3]);                            // S4: K(t,s) R(s,t')
+      acc[6] = fma(f1<PD>(mc, B2C), nR2, acc[6]);               // S7: D(s,t') R(t,s)
+      acc[7] = fma(nR2, f2<PD>(mc, B2C) * B2R, acc[7]);         // S8: R(t,s) K(s,t')
+      // ---- rotate the pipeline ----
+      eA1 = eB1, eA2 = eB2, eA3 = eB3, tnA = tnB;
+      eB1 = eC1, eB2 = eC2, eB3 = eC3, tnB = tnC;
+      n2A = n2B;
+      tau2A = tau2B;
+    }
+    // ---- reduction over j: shuffle within the warp, fixed order across the warps of the group ----
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+      for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
+    if (G > 1) {
+      if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) red[parity][warp][k] = acc[k];
+      }
+      group_barrier(1 + group, TG);  // red[parity] is reused two targets later: one barrier suffices
+    }
+    if (tig != 0) continue;
 
-  // ---- combine (Eq.(1), second-argument equations, Eq.(22)) ----
-  const double mu = a.scal[SC_MU];
-  // mu(theta_i t): local 4-point Lagrange in t over rows k..k+3 (reading G11), mu_M = mu
-  const int npts = (M + 1 < 4) ? M + 1 : 4;
-  int k0 = n1 - 1;
-  if (k0 > M + 1 - npts) k0 = M + 1 - npts;
-  if (k0 < 0) k0 = 0;
-  double mu_p = 0.0;
-  for (int p = 0; p < npts; ++p) {
-    double wgt = 1.0;
-    for (int q = 0; q < npts; ++q)
-      if (q != p) wgt *= (tau1 - a.t[k0 + q]) / (a.t[k0 + p] - a.t[k0 + q]);
-    const double mv = (k0 + p == M) ? mu : a.mu_hist[k0 + p];
-    mu_p += wgt * mv;
-  }
-  const double2 ci = a.cur[i], c0 = a.cur[0];
-  const double fc = mc.beta0 * f1<PD>(mc, c0.x) * b1c_first;
-  const double fc2 = mc.beta0 * f1<PD>(mc, b1c_first) * c0.x;
-  const double d1C = -mu * ci.x + tM * (th_i * Sd[0] + om_i * Sd[1] + th_i * Sd[2]) + fc;
-  const double d1R = -mu * ci.y + tM * (om_i * Sd[3]);
-  const double d2C = -mu_p * ci.x + tM * (th_i * Sd[4] + th_i * Sd[5] + om_i * Sd[6]) + 2.0 * mc.T * ci.y + fc2;
-  const double d2R = mu_p * ci.y - tM * (om_i * Sd[7]);
-  if (a.out.d1C) a.out.d1C[i] = d1C;
-  if (a.out.d1R) a.out.d1R[i] = d1R;
-  if (a.out.d2C) a.out.d2C[i] = d2C;
-  if (a.out.d2R) a.out.d2R[i] = d2R;
-  if (a.out.F) {
-    a.out.F[2 * i] = d1C + th_i * d2C;
-    a.out.F[2 * i + 1] = d1R + th_i * d2R;
-  }
-  if (i == 0) {
-    if (a.out.mu) a.out.mu[0] = mu;
-    if (a.out.energy) a.out.energy[0] = a.scal[SC_E];
+    double Sd[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      double s = acc[k];
+      if (G > 1) {
+        s = 0.0;
+        for (int w = 0; w < G; ++w) s += red[parity][group * G + w][k];
+      }
+      Sd[k] = s;
+      if (a.out.sums) a.out.sums[(size_t)k * L + i] = s;
+    }
+    if (a.out.rows1) a.out.rows1[i] = n1;
+
+    // ---- combine (Eq.(1), second-argument equations, Eq.(22)) ----
+    const double mu = a.scal[SC_MU];
+    // mu(theta_i t): local 4-point Lagrange in t over rows k..k+3 (reading G11), mu_M = mu
+    const int npts = (M + 1 < 4) ? M + 1 : 4;
+    int k0 = n1 - 1;
+    if (k0 > M + 1 - npts) k0 = M + 1 - npts;
+    if (k0 < 0) k0 = 0;
+    double mu_p = 0.0;
+    for (int p = 0; p < npts; ++p) {
+      double wgt = 1.0;
+      for (int q = 0; q < npts; ++q)
+        if (q != p) wgt *= (tau1 - a.t[k0 + q]) / (a.t[k0 + p] - a.t[k0 + q]);
+      const double mv = (k0 + p == M) ? mu : a.mu_hist[k0 + p];
+      mu_p += wgt * mv;
+    }
+    const double2 ci = ld_tab<SM>(cur + i), c0 = ld_tab<SM>(cur);
+    const double fc = mc.beta0 * f1<PD>(mc, c0.x) * b1c_first;
+    const double fc2 = mc.beta0 * f1<PD>(mc, b1c_first) * c0.x;
+    const double d1C = -mu * ci.x + tM * (th_i * Sd[0] + om_i * Sd[1] + th_i * Sd[2]) + fc;
+    const double d1R = -mu * ci.y + tM * (om_i * Sd[3]);
+    const double d2C = -mu_p * ci.x + tM * (th_i * Sd[4] + th_i * Sd[5] + om_i * Sd[6]) + 2.0 * mc.T * ci.y + fc2;
+    const double d2R = mu_p * ci.y - tM * (om_i * Sd[7]);
+    if (a.out.d1C) a.out.d1C[i] = d1C;
+    if (a.out.d1R) a.out.d1R[i] = d1R;
+    if (a.out.d2C) a.out.d2C[i] = d2C;
+    if (a.out.d2R) a.out.d2R[i] = d2R;
+    if (a.out.F) {
+      a.out.F[2 * i] = d1C + th_i * d2C;
+      a.out.F[2 * i + 1] = d1R + th_i * d2R;
+    }
+    if (i == 0) {
+      if (a.out.mu) a.out.mu[0] = mu;
+      if (a.out.energy) a.out.energy[0] = a.scal[SC_E];
+    }
   }
 }
 
@@ -394,7 +522,7 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   a.M = M;
   a.theta = ctx->theta;
   a.omega = ctx->omega;
-  a.nu = ctx->nu;
+  a.thnu = ctx->thnu;
   a.tab = ctx->tab;
   a.t = t;
   a.mu_hist = mu_hist;
@@ -416,8 +544,41 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   // the polynomial degree of f is a compile-time constant for p_max <= 4 (the paper's models
   // p = 2, 3, 2+4, 3+4, 2+3+4); larger p_max (3+9) takes the run-time Horner loop
   const int pd = ctx->model.pmax <= 3 ? 3 : (ctx->model.pmax == 4 ? 4 : 0);
-#define DMFE_LAUNCH(S_, PD_) \
-  history_integrals_kernel<S_, PD_><<<L, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model)
+  // persistent grid: one CTA per SM.  Warps per target group: as few as keeps every warp slot of
+  // the GPU busy (L * G >= resident warps), so that a group's loop over j is as long as possible.
+  const int warps_cta = RHS_THREADS / 32;
+  // G = warps per target group.  As few as possible (long loops over j), subject to (a) every warp
+  // slot of the GPU has work (L * G >= resident warps) and (b) the number of rounds
+  // ceil(L / (groups per CTA * SMs)) wastes less than 3 % of the last round (else the best G).
+  int G = 1;
+  {
+    double best = -1.0;
+    for (int g = 1; g <= warps_cta; g *= 2) {
+      const long long slots = (long long)ctx->sm_count * (warps_cta / g);
+      const long long rounds = ((long long)L + slots - 1) / slots;
+      const double eff = (double)L / (double)(rounds * slots);
+      if (eff > best + 1e-9) best = eff, G = g;
+      if (eff >= 0.97) break;
+    }
+  }
+  a.G = G;
+  const int ngroups = warps_cta / G;
+  int grid = (L + ngroups - 1) / ngroups;
+  if (grid > ctx->sm_count) grid = ctx->sm_count;
+  // shared-memory copies of cur [L] double2, rowtab [M] double2, blo [L] int32 when they fit
+  const size_t smem = 16 * (size_t)L + 16 * (size_t)M + 4 * (size_t)L;
+  const bool sm = smem <= (size_t)ctx->smem_max;
+#define DMFE_LAUNCH(S_, PD_)                                                                              \
+  do {                                                                                                    \
+    if (sm) {                                                                                             \
+      auto kfn = history_integrals_kernel<S_, PD_, true>;                                                 \
+      if (smem > 48 * 1024)                                                                               \
+        CUDA_TRY(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+      kfn<<<grid, RHS_THREADS, smem, ctx->stream>>>(a, ctx->model);                                       \
+    } else {                                                                                              \
+      history_integrals_kernel<S_, PD_, false><<<grid, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model);     \
+    }                                                                                                     \
+  } while (0)
 #define DMFE_LAUNCH_S(S_)        \
   do {                           \
     if (pd == 3)                 \

@@ -220,6 +220,11 @@ int dmfe_build_tables(dmfe_ctx *ctx) {
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->theta, theta.data(), vb, cudaMemcpyHostToDevice, ctx->stream));
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->omega, omega.data(), vb, cudaMemcpyHostToDevice, ctx->stream));
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->nu, nu.data(), vb, cudaMemcpyHostToDevice, ctx->stream));
+  // {theta_j, nu_j} interleaved: the pair kernel reads both with one 16-byte load
+  std::vector<double> thnu(2 * (size_t)L);
+  for (int j = 0; j < L; ++j) thnu[2 * j] = theta[j], thnu[2 * j + 1] = nu[j];
+  CUDA_TRY(ctx, cudaMalloc(&ctx->thnu, 2 * vb));
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->thnu, thnu.data(), 2 * vb, cudaMemcpyHostToDevice, ctx->stream));
   const int nt = 256;
   int gx = (L + nt - 1) / nt;
   if (gx > 64) gx = 64;

@@ -13,7 +13,8 @@ from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_int, c_int32
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libdmfe.so")
+# DMFE_LIBRARY: load another build of the same library (kernel tuning experiments)
+LIB_PATH = os.environ.get("DMFE_LIBRARY") or os.path.join(_HERE, "libdmfe.so")
 
 DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE, DMFE_ENOMEM = 0, -1, -2, -3, -4, -5, -6
 

@@ -156,6 +156,37 @@ def test_rhs_matches_oracle_synthetic(D, L, lo, hi, t_max, lam):
     compare_rhs(g, ref)
 
 
+def test_rhs_full_bench_size_sampled_targets(D):
+    """BASELINE.json config 2 at its full size (L = N = 4096, the launch configuration bench.py
+    times): every output of seeded blocks of targets against the oracle run on those targets."""
+    import torch
+    L, s, t_max, lam = 4096, 4, 1e4, [0, 0, 0, 1.0]
+    ctx = D.dmfe_create(L, s, t_max, lam, T=0.5)
+    try:
+        tab = D.dmfe_get_tables(ctx, L, want_pairs=False)
+        t, mu, hist = inputs.synthetic_history(tab["theta"], tab["omega"], L, -2.0, 4.0)
+        g = gpu_rhs(D, ctx, L, t, mu, hist, L, want_rows=False)
+        rng = np.random.Generator(np.random.PCG64(4096))
+        blocks = np.sort(rng.choice(L // 32, size=8, replace=False)) * 32
+        blocks = np.unique(np.concatenate([[0], blocks, [L - 32]]))
+        grid = _oracle_grid_from_library(tab, L, s, t_max)
+        model = O.Model(np.array(lam, dtype=np.float64), 0.5, 0.0)
+        for i0 in blocks:
+            part = D.dmfe_get_tables(ctx, L, i0=int(i0), n_targets=32)
+            targets = np.arange(i0, i0 + 32, dtype=np.int32)
+            ref = O.history_integrals(grid, model, t, mu, hist, L - 1, targets=targets,
+                                      tables=(part["start"], part["frac"]))
+            err = np.abs(g["sums"].T[targets] - ref["sums"])
+            worst = np.max(err / (RTOL * ref["abssums"] + 1e-300))
+            assert worst <= 1.0, "block %d: sums off by %.3g x tolerance" % (i0, worst)
+            for k, name in enumerate(["d1C", "d1R", "d2C", "d2R"]):
+                e = np.abs(g[name][targets] - ref["deriv"][:, k])
+                assert np.max(e / (RTOL * ref["scale"][:, k] + 1e-300)) <= 1.0, name
+        assert abs(g["mu_out"][0] - ref["mu"]) <= RTOL * abs(ref["mu"])
+    finally:
+        D.dmfe_destroy(ctx)
+
+
 def test_rhs_rows_in_a_larger_buffer(D):
     """n_rows < n_cap: rows beyond the current one are never touched (filled with NaN here)."""
     L, N, s = 80, 20, 4
