@@ -141,6 +141,12 @@ DMFE_API int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int
 DMFE_API int dmfe_sparsify(dmfe_ctx *ctx, dmfe_state *st, int32_t protect_last, int32_t *n_rows_out,
                   uint8_t *keep_mask);
 
+/* Threshold that eps_sparse of Eq.(27) is compared with.  The paper fixes it at tol/10
+ * (PAPER.md:334), which is the default (eps_sparse = 0 restores it).  A caller that must keep the
+ * history below a hard row cap (BASELINE.json configs 3, 4) raises it when a forced pass frees too
+ * little (reading G25 in DESIGN.md); every such change is the caller's and is reported by it. */
+DMFE_API int dmfe_set_sparsify_threshold(dmfe_ctx *ctx, double eps_sparse);
+
 /* Measurement hooks (bench.py).  dmfe_enable_timing: when on, every dmfe_history_integrals launch
  * records CUDA events on the context's stream immediately before and after the pair kernel (the
  * dominant kernel); dmfe_last_kernel_ms synchronises on the closing event and returns the elapsed

@@ -572,7 +572,7 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   do {                                                                                                    \
     if (sm) {                                                                                             \
       auto kfn = history_integrals_kernel<S_, PD_, true>;                                                 \
-      if (smem > 48 * 1024)                                                                               \
+      if (smem + 4096 > 48 * 1024)                                                                        \
         CUDA_TRY(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
       kfn<<<grid, RHS_THREADS, smem, ctx->stream>>>(a, ctx->model);                                       \
     } else {                                                                                              \

@@ -110,6 +110,12 @@ __global__ void sparsify_scatter_kernel(int L, const int32_t *__restrict__ iscal
 
 }  // namespace
 
+extern "C" int dmfe_set_sparsify_threshold(dmfe_ctx *ctx, double eps_sparse) {
+  if (!ctx || !(eps_sparse >= 0.0)) return DMFE_EINVAL;
+  ctx->eps_sparse = eps_sparse;
+  return DMFE_OK;
+}
+
 extern "C" int dmfe_sparsify(dmfe_ctx *ctx, dmfe_state *st, int32_t protect_last, int32_t *n_rows_out,
                              uint8_t *keep_mask) {
   if (!ctx || !st || !st->t || !st->mu || !st->hist || protect_last < 0) return DMFE_EINVAL;
@@ -146,7 +152,7 @@ extern "C" int dmfe_sparsify(dmfe_ctx *ctx, dmfe_state *st, int32_t protect_last
   double4 *tmp_rows = (double4 *)ctx->row_tmp;
   double *tmp_sc = ctx->row_tmp + (size_t)(N - 1) * L * 4;
   sparsify_residual_kernel<<<N - 2, 256, 0, s>>>(L, N, st->t, (const double4 *)st->hist, ctx->eps_sp);
-  sparsify_walk_kernel<<<1, 32, 0, s>>>(N, protect_last, ctx->p.tol / 10.0, ctx->eps_sp, ctx->keep, ctx->newidx,
+  sparsify_walk_kernel<<<1, 32, 0, s>>>(N, protect_last, ctx->eps_sparse > 0.0 ? ctx->eps_sparse : ctx->p.tol / 10.0, ctx->eps_sp, ctx->keep, ctx->newidx,
                                         ctx->iscal);
   const int nb = (N - 1 < 1184) ? N - 1 : 1184;
   sparsify_gather_kernel<<<nb, 128, 0, s>>>(L, ctx->iscal, ctx->newidx, (const double4 *)st->hist, st->t, st->mu,

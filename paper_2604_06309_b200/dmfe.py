@@ -20,7 +20,7 @@ DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE
 
 EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror", "dmfe_get_tables",
            "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_init_state", "dmfe_rk_step",
-           "dmfe_sparsify", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
+           "dmfe_sparsify", "dmfe_set_sparsify_threshold", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
            "dmfe_probe_fp64_tflops"]
 
 
@@ -82,6 +82,8 @@ def load_library():
     lib.dmfe_rk_step.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32)]
     lib.dmfe_sparsify.restype = c_int
     lib.dmfe_sparsify.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32), c_void_p]
+    lib.dmfe_set_sparsify_threshold.restype = c_int
+    lib.dmfe_set_sparsify_threshold.argtypes = [c_void_p, c_double]
     lib.dmfe_enable_timing.restype = c_int
     lib.dmfe_enable_timing.argtypes = [c_void_p, c_int32]
     lib.dmfe_last_kernel_ms.restype = c_int
@@ -203,6 +205,10 @@ def dmfe_sparsify(ctx, st, protect_last=12, want_mask=False):
     mask = np.zeros(st.n_rows, dtype=np.uint8) if want_mask else None
     _check(load_library().dmfe_sparsify(ctx, byref(st), protect_last, byref(n_out), _host(mask)), "dmfe_sparsify", ctx)
     return n_out.value, (mask.astype(bool) if want_mask else None)
+
+
+def dmfe_set_sparsify_threshold(ctx, eps_sparse):
+    _check(load_library().dmfe_set_sparsify_threshold(ctx, float(eps_sparse)), "dmfe_set_sparsify_threshold", ctx)
 
 
 def dmfe_enable_timing(ctx, on=True):
