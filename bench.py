@@ -155,6 +155,29 @@ def oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, n_targets,
     return len(targets), dt
 
 
+# ---- multi-rank host logic (replicas only); covered by a gloo test on CPU ----
+def replica_seed(rank: int) -> int:
+    """Every rank evaluates its own replica: the seed is offset so that the replicas are distinct problems."""
+    from paper_2604_06309_b200 import inputs
+    return inputs.DEFAULT_SEED + 16 * rank
+
+
+def max_over_ranks(ms: float, world: int, device=None) -> float:
+    """Timing of a multi-rank run = the slowest rank (all_reduce MAX; identity for one rank)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(units_per_rank_step: int, steps: int, world: int, ms_total: float) -> float:
+    """Whole-job throughput: the units all ranks processed over the max-over-ranks time."""
+    return units_per_rank_step * steps * world / (ms_total * 1e-3)
+
+
 def host_cores():
     try:
         n = len(os.sched_getaffinity(0))
@@ -225,7 +248,7 @@ def run_ours(args):
     theta, omega, nu = tab["theta"], tab["omega"], tab["nu"]
     # every rank evaluates its own replica of the workload (weak scaling, no data-path collective:
     # DESIGN.md "Multi-GPU"); the seed is offset per rank so that the replicas are distinct problems
-    t, mu, hist = inputs.synthetic_history(theta, omega, N, lo, hi, seed=inputs.DEFAULT_SEED + 16 * rank)
+    t, mu, hist = inputs.synthetic_history(theta, omega, N, lo, hi, seed=replica_seed(rank))
     tt, tm, th = (torch.from_numpy(a).to(dev) for a in (t, mu, hist))
     out = dict(d1C=torch.zeros(L, dtype=torch.float64, device=dev), d1R=torch.zeros(L, dtype=torch.float64, device=dev),
                mu_out=torch.zeros(1, dtype=torch.float64, device=dev),
@@ -257,10 +280,7 @@ def run_ours(args):
     n_k, k_ms, k_min = D.dmfe_kernel_time_stats(ctx)
     D.dmfe_enable_timing(ctx, False)
     clocks = sampler.stop() if sampler else None
-    tmax = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total = float(tmax.item())
+    ms_total = max_over_ranks(ms_total, world, dev)
 
     # ---- end-to-end: host buffers through dmfe_history_integrals_host --------------------------
     ht = torch.from_numpy(t).pin_memory()
@@ -285,10 +305,7 @@ def run_ours(args):
     e2e_ms = max(e0.elapsed_time(e1), 0.0)
     e2e_wall = 1e3 * (time.perf_counter() - w0)
     e2e_ms = max(e2e_ms, e2e_wall if world == 1 else e2e_ms)  # host-synchronous call: wall >= device span
-    tmax = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    e2e_ms = float(tmax.item())
+    e2e_ms = max_over_ranks(e2e_ms, world, dev)
     h2d = int(t.nbytes + mu.nbytes + hist.nbytes)
     d2h = int(2 * L * 8 + 16)
 
@@ -341,7 +358,7 @@ def run_ours(args):
            "sample": "%d seeded targets x %d nodes of the same L=N=%d evaluation (%.1f s)" % (n_s, L, L, dt)}
     D.dmfe_destroy(ctx)
 
-    value = EVALS_PER_PAIR * pairs * args.steps * world / (ms_total * 1e-3)
+    value = job_value(EVALS_PER_PAIR * pairs, args.steps, world, ms_total)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
