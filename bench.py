@@ -141,18 +141,24 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
-def oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, n_targets, seed=12345):
-    """Time the CPU oracle (as it stands) on `n_targets` seeded targets x all L nodes."""
+def oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, n_targets, seed=12345, min_seconds=0.0,
+                  max_reps=64):
+    """Time the CPU oracle (as it stands) on `n_targets` seeded targets x all L nodes; the same
+    evaluation is repeated until `min_seconds` of CPU work have been timed.  Returns (targets per
+    repetition, repetitions, seconds)."""
     from oracle import dmfe_oracle as O
     rng = np.random.Generator(np.random.PCG64(seed))
     targets = np.sort(rng.choice(L, size=min(n_targets, L), replace=False)).astype(np.int32)
     grid = O.Grid(L=L, s=s, t_max=t_max, theta=theta, omega=omega, nu=nu)
     tables = grid.tables(targets)          # table construction is start-up work, not timed
     model = O.Model(np.array(lam, dtype=np.float64), T, 0.0)
-    t0 = time.perf_counter()
-    O.history_integrals(grid, model, t, mu, hist, len(t) - 1, targets=targets, tables=tables)
-    dt = time.perf_counter() - t0
-    return len(targets), dt
+    reps, dt = 0, 0.0
+    while reps < max_reps and (reps == 0 or dt < min_seconds):
+        t0 = time.perf_counter()
+        O.history_integrals(grid, model, t, mu, hist, len(t) - 1, targets=targets, tables=tables)
+        dt += time.perf_counter() - t0
+        reps += 1
+    return len(targets), reps, dt
 
 
 # ---- multi-rank host logic (replicas only, DESIGN.md section 8); covered by a gloo test on CPU ----
@@ -201,10 +207,11 @@ def run_reference(args):
     nt = args.ref_targets
     times = []
     for k in range(args.warmup + args.steps):
-        n, dt = oracle_sample(L, s, t_max, lam, T, grid.theta, grid.omega, grid.nu, t, mu, hist, nt, seed=100 + k)
+        n, reps, dt = oracle_sample(L, s, t_max, lam, T, grid.theta, grid.omega, grid.nu, t, mu, hist, nt, seed=100 + k)
         if k >= args.warmup:
             times.append(dt)
     tot = float(np.sum(times))
+    nt = n
     value = EVALS_PER_PAIR * nt * L * args.steps / tot
     cores = host_cores()
     sample = "%d seeded targets x %d nodes per step of the L=N=%d evaluation" % (nt, L, L)
@@ -340,8 +347,16 @@ def run_ours(args):
     else:
         roof = {"bound": "alu", "achieved": pairs * fpp / (k_avg_ms * 1e-3) / 1e12, "peak": fp64_tf, "unit": "TFLOP/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
+    traffic, traffic_src = args.traffic_bytes, "--traffic-bytes"
+    if traffic is None:
+        try:   # dram bytes per launch of this kernel on this workload from the committed ncu capture
+            tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+            key = "%s_L%d_s%d" % (args.workload, L, s)
+            traffic, traffic_src = tj[key]["dram_bytes_per_launch"], tj[key]["source"]
+        except Exception:
+            traffic, traffic_src = None, None
     roof.update({
-        "traffic": args.traffic_bytes, "peak_source": "hbm: %s copy bandwidth; alu: DFMA chain measured in this run "
+        "traffic": traffic, "traffic_source": traffic_src, "peak_source": "hbm: %s copy bandwidth; alu: DFMA chain measured in this run "
         "on %d SMs" % (hbm_src, sms), "kernel": "history_integrals_kernel<%d>" % s, "kernel_ms_avg": k_avg_ms,
         "kernel_ms_min": k_min, "launches_timed": n_k, "algorithmic_bytes": alg_bytes,
         "algorithmic_bytes_sampled": sampled, "table_bytes": table_bytes, "flops_per_pair": fpp,
@@ -353,10 +368,25 @@ def run_ours(args):
 
     # ---- the oracle on this box's host cores, bounded sample -----------------------------------
     nt = args.ref_targets
-    n_s, dt = oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, nt)
-    cpu = {"value": EVALS_PER_PAIR * n_s * L / dt, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
-           "sample": "%d seeded targets x %d nodes of the same L=N=%d evaluation (%.1f s)" % (n_s, L, L, dt)}
+    n_s, reps, dt = oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, nt, min_seconds=args.ref_seconds)
+    cpu = {"value": EVALS_PER_PAIR * n_s * L * reps / dt, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
+           "sample": "%d seeded targets x %d nodes of the same L=N=%d evaluation, repeated %d times (%.1f s of "
+                     "CPU work)" % (n_s, L, L, reps, dt)}
     D.dmfe_destroy(ctx)
+
+    # ---- adaptive trajectory (BASELINE.json configs[3]): bounded segment, wall time per decade ----
+    traj = None
+    if args.traj_seconds > 0:
+        from paper_2604_06309_b200 import trajectory
+        cfg = dict(trajectory.CONFIGS[4])
+        out = trajectory.run(t_end=1e7, max_seconds=args.traj_seconds, **cfg)
+        stt = out["stats"]
+        traj = {"workload": "config4: pure 3-spin aging run, T=0.5, tol=1e-8, L=%d, s=%d, n_cap=%d, first %.0f s of "
+                            "wall time" % (cfg["L"], cfg["s"], cfg["n_cap"], args.traj_seconds),
+                "steps_per_s": stt["steps"] / stt["wall_s"], "rhs_per_s": stt["n_rhs"] / stt["wall_s"],
+                "t_reached": stt["t_reached"], "wall_s_to_t": out["wall_to_t"], "reverted": stt["reverted"],
+                "n_rows": stt["n_rows"], "status": stt["status"],
+                "full_runs": "profiles/ holds the wall times of the runs to t=1e5 (config 3) and t=1e7 (config 4)"}
 
     value = job_value(EVALS_PER_PAIR * pairs, args.steps, world, ms_total)
     line = {
@@ -373,6 +403,7 @@ def run_ours(args):
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
                 "ms_per_step": e2e_ms / e2e_steps},
         "gpu_launches": 2 * args.steps,
+        "trajectory": traj,
     }
     print(json.dumps(line))
     if world > 1:
@@ -390,7 +421,10 @@ def main():
     ap.add_argument("--L", type=int, default=4096)
     ap.add_argument("--stencil", type=int, default=4)
     ap.add_argument("--ref-targets", type=int, default=4096, help="targets per oracle sample")
+    ap.add_argument("--ref-seconds", type=float, default=10.0, help="CPU time of the oracle sample in the ours arm")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--traj-seconds", type=float, default=8.0,
+                    help="wall-time budget of the adaptive trajectory segment (0 = skip)")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="dram bytes per launch of the pair kernel from the committed ncu capture (profiles/)")
     args = ap.parse_args()

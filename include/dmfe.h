@@ -160,6 +160,13 @@ DMFE_API int dmfe_last_kernel_ms(dmfe_ctx *ctx, float *ms);
  * launches themselves, so this can bracket every launch of a timed region. */
 DMFE_API int dmfe_kernel_time_stats(dmfe_ctx *ctx, int32_t *n_launches, double *total_ms, double *min_ms);
 DMFE_API int dmfe_probe_fp64_tflops(dmfe_ctx *ctx, int32_t n_iter, double *tflops, int32_t *sm_count);
+/* Load-path probe: one CTA of `threads` threads per SM; per iteration every
+ * warp issues n_loads independent 256-bit loads from an L1-resident buffer with lane pattern
+ * 0 coalesced, 1 lane pairs share a cell, 2 broadcast, 3 stencil-like (cell l/4 + (l&3)), 4 one cell
+ * per 128-byte line, and n_dfma (multiple of 8) independent DFMAs.  Returns SM cycles per
+ * warp-iteration (clock64 around the loop, averaged over SMs).  Synchronises. */
+DMFE_API int dmfe_probe_load_path(dmfe_ctx *ctx, int32_t pattern, int32_t n_loads, int32_t n_dfma, int32_t threads,
+                         double *cycles_per_warp_iter);
 
 #ifdef __cplusplus
 }

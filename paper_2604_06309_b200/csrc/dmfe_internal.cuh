@@ -29,7 +29,8 @@ enum {
   SC_H = 2,      // current step size
   SC_EPS = 3,    // eps_RK of the last attempted step (Eq.(25))
   SC_T0 = 4,     // t_N at the start of the step
-  SC_HNEXT = 5,  // step size proposed by the controller
+  SC_HNEXT = 5,  // step size proposed by the controller (latched into SC_H by stage 0 of the next step)
+  SC_ACCEPT = 6, // accept flag of the last step as a double (so that one copy returns the whole record)
   SC_COUNT = 16
 };
 // device int block (ctx->iscal)
@@ -120,8 +121,24 @@ DMFE_HD void dmfe_tab_decode(uint64_t e, int32_t *start, double *frac) {
   *frac = x * 16.0 - 257.0;  // exact: x has at most 48 significant fraction bits below 2^4
 }
 
+// One SSPRK(10,4) stage update fused into the O(L + M) pre-pass of the right-hand side that follows
+// it (rk_step.cu fills this in; k < 0 = no stage update, plain evaluation of row M).
+struct dmfe_stage {
+  int32_t k;           // stage 0..9 of PAPER.md:314-316; the update writes the value slots of row N+1
+  int32_t N;           // last complete row
+  int32_t fixed_step;  // k == 9: 1 = no controller
+  double tol, cap;     // k == 9: epsilon of Eq.(25), step cap of Eq.(24)
+  double *hist, *t;    // writable views of the caller's history
+  double *rk;          // [4][2L]: q1, q2, delta, F
+  double *scal;
+  int32_t *iscal;
+};
+
 // tables.cu
 int dmfe_build_tables(dmfe_ctx *ctx);
 // history_integrals.cu
+// stage: optional stage update run by the pre-pass; deriv_row: optional row of the history whose
+// derivative slots receive F (the derivative is stored with the appended row)
 int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, const double *mu_hist,
-                    const double *hist, const dmfe_rhs_out *out);
+                    const double *hist, const dmfe_rhs_out *out, const dmfe_stage *stage = nullptr,
+                    double *deriv_row = nullptr);

@@ -49,6 +49,7 @@ struct RhsArgs {
   const int32_t *blo;
   const double *scal;  // SC_MU, SC_E written by prepare_kernel
   int32_t G;           // warps per target group
+  double4 *deriv_row;  // optional: row of the history whose derivative slots receive F
   dmfe_rhs_out out;
 };
 
@@ -153,25 +154,50 @@ __device__ __forceinline__ void t_weights(double tn, double rD, double tau, bool
 }
 
 // ---------------------------------------------------------------------------------------------
-// O(L + M) pre-pass.  Block 0: pack row M into {C,R} pairs and reduce mu(t) (Eq.(13)) and E(t)
-// (Eq.(14)).  Blocks >= 1 (or block 0 too when launched alone): the per-call row table
-// rowtab[n] = {t_n, 1/(t_{n+1} - t_n)}, n < M, and the bracket table blo[c] = n(fl(theta_c t_M)):
-// for theta_a <= phi < theta_b rounding is monotone, so n(fl(phi t_M)) lies in [blo[a], blo[b]].
-__global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, ModelCoef mc,
+// O(L + M) pre-pass, optionally preceded by one SSPRK(10,4) stage update that
+// produces the row to be evaluated.  Low-storage form (refs [64,65]):
+//   q1 = q2 = y;  5 x { q1 += h/6 F(q1) };  q2 = q2/25 + 9/25 q1;  q1 = 15 q2 - 5 q1;
+//   4 x { q1 += h/6 F(q1) };  y+ = q2 + 3/5 q1 + h/10 F(q1)
+// stage times t + c_k h, c = (0,1,2,3,4,2,3,4,5,6)/6; embedded 3rd-order weights
+// bhat = (0,2/9,0,0,5/18,1/3,0,0,0,1/6) (reading G22); delta = h sum (b_k - bhat_k) F_k.
+// Block 0: stage update of the 2L state entries (stage k = 9 also reduces eps_RK of Eq.(25) and
+// runs the controller of PAPER.md:320, reading G20), then packs row M into {C,R} pairs and
+// reduces mu(t) (Eq.(13)) and E(t) (Eq.(14)).  Blocks >= 1 (or block 0 too when launched alone):
+// the per-call row table rowtab[n] = {t_n, 1/(t_{n+1} - t_n)}, n < M, and the bracket table
+// blo[c] = n(fl(theta_c t_M)): for theta_a <= phi < theta_b rounding is monotone, so
+// n(fl(phi t_M)) lies in [blo[a], blo[b]].  They compute t_M from the step scalars instead of
+// reading t[M], which block 0 is writing.
+__constant__ double c_stage_c[10] = {0.0,       1.0 / 6.0, 2.0 / 6.0, 3.0 / 6.0, 4.0 / 6.0,
+                                     2.0 / 6.0, 3.0 / 6.0, 4.0 / 6.0, 5.0 / 6.0, 6.0 / 6.0};
+__constant__ double c_b_minus_bhat[10] = {0.1 - 0.0, 0.1 - 2.0 / 9.0, 0.1 - 0.0, 0.1 - 0.0, 0.1 - 5.0 / 18.0,
+                                          0.1 - 1.0 / 3.0, 0.1 - 0.0, 0.1 - 0.0, 0.1 - 0.0, 0.1 - 1.0 / 6.0};
+
+__global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, ModelCoef mc, dmfe_stage sg,
                                                                const double *__restrict__ theta,
-                                                               const double *__restrict__ nu,
-                                                               const double *__restrict__ t,
-                                                               const double4 *__restrict__ hist,
-                                                               double2 *__restrict__ cur, double2 *__restrict__ rowtab,
-                                                               int32_t *__restrict__ blo, double *__restrict__ scal) {
+                                                               const double *__restrict__ nu, const double *t,
+                                                               const double4 *hist, double2 *__restrict__ cur,
+                                                               double2 *__restrict__ rowtab,
+                                                               int32_t *__restrict__ blo, double *scal) {
+  __shared__ double sm[32], se[32];
+  const int k = sg.k;
+  // time of the row being evaluated.  The step size of stage 0 is the controller's proposal
+  // (SC_HNEXT); block 0 latches it into SC_H, which stages 1..9 read.
+  double tM, h = 0.0;
+  if (k >= 0) {
+    h = (k == 0) ? scal[SC_HNEXT] : scal[SC_H];
+    const double t0 = t[sg.N];
+    tM = (k < 9) ? __dadd_rn(t0, __dmul_rn(c_stage_c[k + 1], h)) : __dadd_rn(t0, h);
+  } else {
+    tM = t[M];
+  }
   if (blockIdx.x > 0 || gridDim.x == 1) {
     const int nb = gridDim.x == 1 ? 1 : gridDim.x - 1;
     const int b = gridDim.x == 1 ? 0 : blockIdx.x - 1;
-    const double tM = t[M];
     for (int e = b * PREP_THREADS + threadIdx.x; e < M + L; e += nb * PREP_THREADS) {
       if (e < M) {
         const double tn = t[e];
-        rowtab[e] = make_double2(tn, 1.0 / (t[e + 1] - tn));
+        const double tn1 = (e + 1 == M) ? tM : t[e + 1];
+        rowtab[e] = make_double2(tn, 1.0 / (tn1 - tn));
       } else {
         const int c = e - M;
         blo[c] = row_search(t, 0, M - 1, __dmul_rn(theta[c], tM));
@@ -179,11 +205,82 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
     }
     if (blockIdx.x > 0) return;
   }
-  __shared__ double sm[32], se[32];
+  if (k >= 0) {
+    // ---- stage update: rk = [4][2L]: q1, q2, delta, F ----
+    const int n2 = 2 * L, N = sg.N;
+    double *q1 = sg.rk, *q2 = sg.rk + n2, *dl = sg.rk + 2 * n2;
+    const double *F = sg.rk + 3 * n2;
+    const double hb = __dmul_rn(h, c_b_minus_bhat[k]);
+    const double h6 = h / 6.0;
+    double eacc = 0.0;
+    for (int e = threadIdx.x; e < n2; e += blockDim.x) {
+      const int l = e >> 1, comp = e & 1;
+      const size_t cellN = ((size_t)N * L + l) * 4, cellM = ((size_t)M * L + l) * 4;
+      double a, b, d, Fk;
+      if (k == 0) {
+        a = b = sg.hist[cellN + 2 * comp];
+        d = 0.0;
+        Fk = sg.hist[cellN + 2 * comp + 1];
+      } else {
+        a = q1[e];
+        b = q2[e];
+        d = dl[e];
+        Fk = F[e];
+      }
+      d = __dadd_rn(d, __dmul_rn(hb, Fk));
+      if (k < 9) {
+        a = __dadd_rn(a, __dmul_rn(h6, Fk));
+        if (k == 4) {
+          b = __dadd_rn(b / 25.0, __dmul_rn(9.0 / 25.0, a));
+          a = __dsub_rn(__dmul_rn(15.0, b), __dmul_rn(5.0, a));
+        }
+      } else {
+        a = __dadd_rn(__dadd_rn(b, __dmul_rn(0.6, a)), __dmul_rn(__dmul_rn(0.1, h), Fk));
+        eacc += fabs(d);
+      }
+      q1[e] = a;
+      q2[e] = b;
+      dl[e] = d;
+      sg.hist[cellM + 2 * comp] = a;  // stage state = value slots of the current row M
+    }
+    if (threadIdx.x == 0) {
+      sg.t[M] = tM;
+      if (k == 0) scal[SC_H] = h;
+    }
+    if (k == 9) {
+      // eps_RK = sum_i |delta C_i| + |delta R_i| (Eq.(25)) and the controller (G20)
+      for (int o = 16; o > 0; o >>= 1) eacc += __shfl_xor_sync(0xffffffffu, eacc, o);
+      if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = eacc;
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        double eps = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) eps += sm[w];
+        double hn = h;
+        int accept = 1;
+        if (!sg.fixed_step) {
+          if (!isfinite(eps) || eps > 2.0 * sg.tol) {
+            accept = 0;
+            hn = fmin(h / 2.0, sg.cap);
+          } else {
+            if (eps > sg.tol)
+              hn = 0.9 * h;
+            else if (eps < sg.tol / 2.0)
+              hn = 1.01 * h;
+            hn = fmin(hn, sg.cap);
+          }
+        }
+        scal[SC_EPS] = eps;
+        scal[SC_HNEXT] = hn;
+        scal[SC_ACCEPT] = (double)accept;
+        sg.iscal[IS_ACCEPT] = accept;
+      }
+    }
+    __syncthreads();  // the row written above is read below by other threads of this block
+  }
   const double4 *row = hist + (size_t)M * (size_t)L;
   double am = 0.0, ae = 0.0;
   for (int j = threadIdx.x; j < L; j += blockDim.x) {
-    const double4 c = ld_cell(row + j);
+    const double4 c = row[j];  // plain load: the value slots may have been written by this block
     cur[j] = make_double2(c.x, c.z);
     const double fp = horner(mc.c1, mc.pmax - 1, c.x), fpp = horner(mc.c2, mc.pmax - 2, c.x);
     const double nj = nu[j];
@@ -195,19 +292,18 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
     ae += __shfl_xor_sync(0xffffffffu, ae, o);
   }
   const int w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  __syncthreads();  // sm[] may still be read by thread 0 (stage 9)
   if ((threadIdx.x & 31) == 0) sm[w] = am, se[w] = ae;
   __syncthreads();
   if (threadIdx.x == 0) {
     double tm = 0.0, te = 0.0;
-    for (int k = 0; k < nw; ++k) tm += sm[k], te += se[k];
-    const double tM = t[M];
+    for (int q = 0; q < nw; ++q) tm += sm[q], te += se[q];
     const double c0 = row[0].x;
     scal[SC_MU] = mc.T + tM * tm + mc.beta0 * horner(mc.c1, mc.pmax - 1, c0) * c0;
     scal[SC_E] = -tM * te - mc.beta0 * horner(mc.c0, mc.pmax, c0);
   }
 }
 
-// ---------------------------------------------------------------------------------------------
 // Small per-call tables (current row, row table, bracket table) live in shared memory when they
 // fit (SM = true): the gathers into them are the head of every pair's dependent load chain, and
 // the history cells streaming through L1 (1 KB per warp-wide load) would otherwise evict them
@@ -235,7 +331,7 @@ __device__ __forceinline__ int row_search_tab(const double2 *rowtab, int lo, int
 // row n2, found by bisection inside the bracket of the grid cell of phi2.  l* = max{l : theta_l <=
 // phi2} equals a2 + S/2 - 1 unless the stencil start was clamped, in which case l* lies in
 // [0, S/2-1] (a2 = 0) or [L-S/2-1, L-1] (a2 = L-S).  n2 <= M-1, so the search runs on rowtab[0..M-1].
-template <int S, bool SM>
+template <int S, bool SMT, bool SMR>
 __device__ __forceinline__ int index_stage(const double2 *rowtab, const int32_t *blo, const double4 *hist, int L,
                                            double th_i, double om_i, double tM, double th_j, int a2, int a3,
                                            double *tau2_out) {
@@ -244,7 +340,7 @@ __device__ __forceinline__ int index_stage(const double2 *rowtab, const int32_t 
   int clo = a2 + (S / 2 - 1), chi = clo + 1;
   if (a2 == 0) clo = 0, chi = S / 2;
   if (a2 == L - S) clo = (a2 == 0) ? 0 : L - S / 2 - 1, chi = L - 1;
-  const int n2 = row_search_tab<SM>(rowtab, ld_tab<SM>(blo + clo), ld_tab<SM>(blo + chi), tau2);
+  const int n2 = row_search_tab<SMR>(rowtab, ld_tab<SMT>(blo + clo), ld_tab<SMT>(blo + chi), tau2);
   *tau2_out = tau2;
   return n2;
 }
@@ -255,21 +351,25 @@ __device__ __forceinline__ void group_barrier(int id, int nthreads) {
 
 // Persistent kernel: one CTA per SM; the CTA's warps form groups of G warps, a group evaluates one
 // target i at a time (lanes <-> adjacent nodes j), groups of one CTA take adjacent targets.
-template <int S, int PD, bool SM>
+// SM: 0 = per-call tables read from global memory, 1 = cur and blo in shared memory, 2 = rowtab too
+template <int S, int PD, int SM>
 __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
+  constexpr bool SMT = SM >= 1, SMR = SM == 2;
   extern __shared__ double4 smem_dyn[];
   const int L = a.L, M = a.M;
   const double2 *cur = a.cur;
   const double2 *rowtab = a.rowtab;
   const int32_t *blo = a.blo;
-  if (SM) {
+  if (SMT) {
     double2 *s_cur = reinterpret_cast<double2 *>(smem_dyn);
     double2 *s_row = s_cur + L;
-    int32_t *s_blo = reinterpret_cast<int32_t *>(s_row + M);
+    int32_t *s_blo = reinterpret_cast<int32_t *>(s_row + (SMR ? M : 0));
     for (int k = threadIdx.x; k < L; k += RHS_THREADS) s_cur[k] = a.cur[k], s_blo[k] = a.blo[k];
-    for (int k = threadIdx.x; k < M; k += RHS_THREADS) s_row[k] = a.rowtab[k];
+    if (SMR)
+      for (int k = threadIdx.x; k < M; k += RHS_THREADS) s_row[k] = a.rowtab[k];
     __syncthreads();
-    cur = s_cur, rowtab = s_row, blo = s_blo;
+    cur = s_cur, blo = s_blo;
+    if (SMR) rowtab = s_row;
   }
   __shared__ double red[2][RHS_THREADS / 32][8];
 
@@ -288,11 +388,11 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
     const double th_i = a.theta[i], om_i = a.omega[i];
     // type-1: one row search per target, tau = theta_i t  (Eq.(19)); blo[i] is exactly that row
     const double tau1 = __dmul_rn(th_i, tM);
-    const int n1 = ld_tab<SM>(blo + i);
+    const int n1 = ld_tab<SMT>(blo + i);
     const bool top1 = (n1 + 1 == M);
     double h1[4];
     {
-      const double2 rt = ld_tab<SM>(rowtab + n1);
+      const double2 rt = ld_tab<SMR>(rowtab + n1);
       t_weights(rt.x, rt.y, tau1, top1, h1);
     }
     const double4 *row1lo = a.hist + (size_t)n1 * (size_t)L;
@@ -324,7 +424,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       tnB = __ldg(a.thnu + j + TG);
     }
     if (j < L)
-      n2A = index_stage<S, SM>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnA.x, (int)(eA2 >> 48), (int)(eA3 >> 48),
+      n2A = index_stage<S, SMT, SMR>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnA.x, (int)(eA2 >> 48), (int)(eA3 >> 48),
                                &tau2A);
     for (; j < L; j += TG) {
       uint64_t eC1 = 0, eC2 = 0, eC3 = 0;
@@ -353,7 +453,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       int n2B = 0;
       double tau2B = 0.0;
       if (j + TG < L)
-        n2B = index_stage<S, SM>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnB.x, (int)(eB2 >> 48),
+        n2B = index_stage<S, SMT, SMR>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnB.x, (int)(eB2 >> 48),
                                  (int)(eB3 >> 48), &tau2B);
 
       const double nj = tnA.y;
@@ -369,7 +469,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         lagrange_weights<S>(u1, w);
 #pragma unroll
         for (int l = 0; l < S; ++l) {
-          const double2 v = ld_tab<SM>(cur + a1 + l);
+          const double2 v = ld_tab<SMT>(cur + a1 + l);
           C1 = fma(w[l], v.x, C1);
           R1 = fma(w[l], v.y, R1);
         }
@@ -387,7 +487,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       lagrange_weights<S>(u2, w);
 #pragma unroll
       for (int l = 0; l < S; ++l) {
-        const double2 v = ld_tab<SM>(cur + a2 + l);
+        const double2 v = ld_tab<SMT>(cur + a2 + l);
         C2 = fma(w[l], v.x, C2);
         R2 = fma(w[l], v.y, R2);
       }
@@ -396,7 +496,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       const bool top2 = (n2 + 1 == M);
       double h2[4];
       {
-        const double2 rt = ld_tab<SM>(rowtab + n2);
+        const double2 rt = ld_tab<SMR>(rowtab + n2);
         t_weights(rt.x, rt.y, tau2A, top2, h2);
       }
       // theta-stencil first, then t
@@ -475,7 +575,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       const double mv = (k0 + p == M) ? mu : a.mu_hist[k0 + p];
       mu_p += wgt * mv;
     }
-    const double2 ci = ld_tab<SM>(cur + i), c0 = ld_tab<SM>(cur);
+    const double2 ci = ld_tab<SMT>(cur + i), c0 = ld_tab<SMT>(cur);
     const double fc = mc.beta0 * f1<PD>(mc, c0.x) * b1c_first;
     const double fc2 = mc.beta0 * f1<PD>(mc, b1c_first) * c0.x;
     const double d1C = -mu * ci.x + tM * (th_i * Sd[0] + om_i * Sd[1] + th_i * Sd[2]) + fc;
@@ -486,9 +586,15 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
     if (a.out.d1R) a.out.d1R[i] = d1R;
     if (a.out.d2C) a.out.d2C[i] = d2C;
     if (a.out.d2R) a.out.d2R[i] = d2R;
+    const double FC = d1C + th_i * d2C, FR = d1R + th_i * d2R;
     if (a.out.F) {
-      a.out.F[2 * i] = d1C + th_i * d2C;
-      a.out.F[2 * i + 1] = d1R + th_i * d2R;
+      a.out.F[2 * i] = FC;
+      a.out.F[2 * i + 1] = FR;
+    }
+    if (a.deriv_row) {  // the ray derivative is stored with the appended row
+      double *cell = reinterpret_cast<double *>(a.deriv_row + i);
+      cell[1] = FC;
+      cell[3] = FR;
     }
     if (i == 0) {
       if (a.out.mu) a.out.mu[0] = mu;
@@ -501,7 +607,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
 
 // M = index of the current row; its time t[M] is read on the device (the RK step keeps t there).
 int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, const double *mu_hist,
-                    const double *hist, const dmfe_rhs_out *out) {
+                    const double *hist, const dmfe_rhs_out *out, const dmfe_stage *stage, double *deriv_row) {
   const int L = ctx->p.L;
   if (M > ctx->rowtab_cap) {  // per-call row table: sized by the caller's capacity, grown on demand
     const int cap = n_cap > M ? n_cap : M;
@@ -514,7 +620,14 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   }
   int pb = 1 + (M + L + PREP_THREADS - 1) / PREP_THREADS;
   if (pb > 17) pb = 17;
-  prepare_kernel<<<pb, PREP_THREADS, 0, ctx->stream>>>(L, M, ctx->model, ctx->theta, ctx->nu, t,
+  dmfe_stage sg;
+  if (stage) {
+    sg = *stage;
+  } else {
+    memset(&sg, 0, sizeof(sg));
+    sg.k = -1;
+  }
+  prepare_kernel<<<pb, PREP_THREADS, 0, ctx->stream>>>(L, M, ctx->model, sg, ctx->theta, ctx->nu, t,
                                                        (const double4 *)hist, ctx->cur, ctx->rowtab, ctx->blo,
                                                        ctx->scal);
   RhsArgs a;
@@ -531,6 +644,7 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   a.rowtab = ctx->rowtab;
   a.blo = ctx->blo;
   a.scal = ctx->scal;
+  a.deriv_row = reinterpret_cast<double4 *>(deriv_row);
   a.out = *out;
   const bool timed = ctx->timing_on && ctx->ev_n < DMFE_EV_RING;
   if (timed) {
@@ -553,7 +667,8 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   int G = 1;
   {
     double best = -1.0;
-    for (int g = 1; g <= warps_cta; g *= 2) {
+    for (int g = 1; g <= warps_cta && g <= 16; g *= 2) {
+      if (warps_cta % g) continue;
       const long long slots = (long long)ctx->sm_count * (warps_cta / g);
       const long long rounds = ((long long)L + slots - 1) / slots;
       const double eff = (double)L / (double)(rounds * slots);
@@ -565,19 +680,28 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   const int ngroups = warps_cta / G;
   int grid = (L + ngroups - 1) / ngroups;
   if (grid > ctx->sm_count) grid = ctx->sm_count;
-  // shared-memory copies of cur [L] double2, rowtab [M] double2, blo [L] int32 when they fit
-  const size_t smem = 16 * (size_t)L + 16 * (size_t)M + 4 * (size_t)L;
-  const bool sm = smem <= (size_t)ctx->smem_max;
-#define DMFE_LAUNCH(S_, PD_)                                                                              \
-  do {                                                                                                    \
-    if (sm) {                                                                                             \
-      auto kfn = history_integrals_kernel<S_, PD_, true>;                                                 \
-      if (smem + 4096 > 48 * 1024)                                                                        \
-        CUDA_TRY(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-      kfn<<<grid, RHS_THREADS, smem, ctx->stream>>>(a, ctx->model);                                       \
-    } else {                                                                                              \
-      history_integrals_kernel<S_, PD_, false><<<grid, RHS_THREADS, 0, ctx->stream>>>(a, ctx->model);     \
-    }                                                                                                     \
+  // shared-memory copies of cur [L] double2 and blo [L] int32 when they fit, and of rowtab [M]
+  // double2 too when that fits and a CTA has enough pairs to amortise copying M entries
+  const size_t smem1 = 20 * (size_t)L, smem2 = smem1 + 16 * (size_t)M;
+  const long long pairs_cta = (long long)L * L / grid;
+  const int mode = (smem2 <= (size_t)ctx->smem_max && 2LL * M <= pairs_cta) ? 2
+                   : (smem1 <= (size_t)ctx->smem_max ? 1 : 0);
+  const size_t smem = mode == 2 ? smem2 : (mode == 1 ? smem1 : 0);
+#define DMFE_LAUNCH_M(S_, PD_, SM_)                                                                     \
+  do {                                                                                                  \
+    auto kfn = history_integrals_kernel<S_, PD_, SM_>;                                                  \
+    if (smem + 4096 > 48 * 1024)                                                                        \
+      CUDA_TRY(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+    kfn<<<grid, RHS_THREADS, smem, ctx->stream>>>(a, ctx->model);                                       \
+  } while (0)
+#define DMFE_LAUNCH(S_, PD_)       \
+  do {                             \
+    if (mode == 2)                 \
+      DMFE_LAUNCH_M(S_, PD_, 2);   \
+    else if (mode == 1)            \
+      DMFE_LAUNCH_M(S_, PD_, 1);   \
+    else                           \
+      DMFE_LAUNCH_M(S_, PD_, 0);   \
   } while (0)
 #define DMFE_LAUNCH_S(S_)        \
   do {                           \
@@ -598,6 +722,7 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   }
 #undef DMFE_LAUNCH_S
 #undef DMFE_LAUNCH
+#undef DMFE_LAUNCH_M
   if (timed) {
     CUDA_TRY(ctx, cudaEventRecord(ctx->ev[2 * ctx->ev_n + 1], ctx->stream));
     ctx->ev_n++;

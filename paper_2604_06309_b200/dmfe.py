@@ -21,7 +21,7 @@ DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE
 EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror", "dmfe_get_tables",
            "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_init_state", "dmfe_rk_step",
            "dmfe_sparsify", "dmfe_set_sparsify_threshold", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
-           "dmfe_probe_fp64_tflops"]
+           "dmfe_probe_fp64_tflops", "dmfe_probe_load_path"]
 
 
 class dmfe_params(Structure):
@@ -84,6 +84,8 @@ def load_library():
     lib.dmfe_sparsify.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32), c_void_p]
     lib.dmfe_set_sparsify_threshold.restype = c_int
     lib.dmfe_set_sparsify_threshold.argtypes = [c_void_p, c_double]
+    lib.dmfe_probe_load_path.restype = c_int
+    lib.dmfe_probe_load_path.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_int32, POINTER(c_double)]
     lib.dmfe_enable_timing.restype = c_int
     lib.dmfe_enable_timing.argtypes = [c_void_p, c_int32]
     lib.dmfe_last_kernel_ms.restype = c_int
@@ -226,6 +228,14 @@ def dmfe_kernel_time_stats(ctx):
     n, tot, mn = c_int32(0), c_double(0.0), c_double(0.0)
     _check(load_library().dmfe_kernel_time_stats(ctx, byref(n), byref(tot), byref(mn)), "dmfe_kernel_time_stats", ctx)
     return n.value, tot.value, mn.value
+
+
+def dmfe_probe_load_path(ctx, pattern, n_loads, n_dfma, threads=512):
+    """-> SM cycles per warp-iteration of the load-path probe (include/dmfe.h)."""
+    out = c_double(0.0)
+    _check(load_library().dmfe_probe_load_path(ctx, pattern, n_loads, n_dfma, threads, byref(out)),
+           "dmfe_probe_load_path", ctx)
+    return out.value
 
 
 def dmfe_probe_fp64_tflops(ctx, n_iter=1 << 16):

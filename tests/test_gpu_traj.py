@@ -184,3 +184,21 @@ def test_sparsify_on_synthetic_rows(D):
     assert n_after == keep_ref.sum()
     assert np.array_equal(got[0], t[keep_ref]) and np.array_equal(got[1], mu[keep_ref])
     assert np.array_equal(got[3], hist[keep_ref])
+
+
+def test_trajectory_driver_with_row_cap(D):
+    """The adaptive driver (paper_2604_06309_b200/trajectory.py) under a hard row cap: periodic
+    sparsification, threshold doubling when a forced pass frees too little (G25), constraints kept."""
+    from paper_2604_06309_b200 import trajectory
+    out = trajectory.run(L=64, s=4, t_max=200.0, lam=[0, 0, 0, 1.0], T=0.5, tol=1e-6, n_cap=120, t_end=60.0,
+                         sp_every=50, n_obs=8, t_w=(1.0, 10.0))
+    st = out["stats"]
+    assert st["status"] == "ok" and st["t_reached"] >= 60.0
+    assert st["n_rows"] <= 120 and st["threshold_doublings"] >= 1
+    assert st["C_diag_drift"] < 1e-12 and st["R_diag_drift"] < 1e-12
+    rec = out["records"]
+    assert len(rec["t"]) >= 4 and all(np.isfinite(rec["E"]))
+    # energy relaxes monotonically towards the aging value after the initial transient (P9 band)
+    assert -0.95 < rec["E"][-1] < -0.6
+    assert 1.0 in rec["corr"][-1] and 0.0 < rec["corr"][-1][1.0][0] < 1.0
+    assert set(out["wall_to_t"]) >= {"1", "10"}
