@@ -117,6 +117,20 @@ __device__ __forceinline__ void lagrange_weights(double u, double (&w)[S]) {
   }
 }
 
+// S = 4: with A = u(u-3) and B = (u-1)(u-2) = A + 2 the four cardinal cubics are
+//   w0 = B(3-u)/6, w1 = A(u-2)/2, w2 = A(1-u)/2, w3 = B u/6      (10 FP64 instructions)
+template <>
+__device__ __forceinline__ void lagrange_weights<4>(double u, double (&w)[4]) {
+  const double A = u * (u - 3.0);
+  const double B = A + 2.0;
+  const double hA = 0.5 * A;
+  const double t6 = u * (1.0 / 6.0);
+  w[3] = B * t6;
+  w[0] = fma(-B, t6, 0.5 * B);
+  w[1] = fma(hA, u, -A);
+  w[2] = fma(-hA, u, hA);
+}
+
 // n = max{ n in [lo, hi] : t[n] <= tau }; requires t[lo] <= tau.
 __device__ __forceinline__ int row_search(const double *__restrict__ t, int lo, int hi, double tau) {
   while (lo < hi) {
@@ -477,10 +491,12 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
         const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
         if (j == 0) b1c_first = B1C;
-        acc[0] = fma(nj * (f2<PD>(mc, C1) * R1), B1C, acc[0]);   // S1: K(t,s) C(t',s)
-        acc[2] = fma(nj * f1<PD>(mc, C1), B1R, acc[2]);          // S3: D(t,s) R(t',s)
-        acc[4] = fma(nj * (f2<PD>(mc, B1C) * B1R), C1, acc[4]);  // S5: K(t',s) C(t,s)
-        acc[5] = fma(nj * f1<PD>(mc, B1C), R1, acc[5]);          // S6: D(t',s) R(t,s)
+        // every term carries nu_j and exactly one of R1, B1R: fold nu_j into those two
+        const double nR1 = nj * R1, nB1R = nj * B1R;
+        acc[0] = fma(f2<PD>(mc, C1) * nR1, B1C, acc[0]);    // S1: K(t,s) C(t',s)
+        acc[2] = fma(f1<PD>(mc, C1), nB1R, acc[2]);         // S3: D(t,s) R(t',s)
+        acc[4] = fma(f2<PD>(mc, B1C) * nB1R, C1, acc[4]);   // S5: K(t',s) C(t,s)
+        acc[5] = fma(f1<PD>(mc, B1C), nR1, acc[5]);         // S6: D(t',s) R(t,s)
       }
       // ---- A factors at phi2 (Eq.(18)) ----
       double C2 = 0.0, R2 = 0.0;

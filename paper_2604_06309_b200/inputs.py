@@ -28,34 +28,37 @@ def log_times(N: int, lo: float, hi: float) -> np.ndarray:
 
 
 def synthetic_history(theta: np.ndarray, omega: np.ndarray, N: int, lo: float, hi: float,
-                      seed: int = DEFAULT_SEED, jitter: float = 1e-6, rows=None):
-    """Returns (t[N], mu[N], hist[N, L, 4]) with hist[..., :] = {C, dC, R, dR}.
-
-    `rows` (optional slice) limits which rows of `hist` are materialised (the jitter stream is
-    still consumed row-major so that any sub-block equals the same block of the full array)."""
+                      seed: int = DEFAULT_SEED, jitter: float = 1e-6):
+    """Returns (t[N], mu[N], hist[N, L, 4]) with hist[..., :] = {C, dC, R, dR}."""
     L = len(theta)
     t = log_times(N, lo, hi)
     mu = 1.0 + 1.0 / (1.0 + t)
     hist = np.empty((N, L, 4), dtype=np.float64)
-    tn = t[:, None]
-    th = theta[None, :]
-    om = omega[None, :]
-    x = th * tn                       # t' = theta t
-    tau = 1.0 + x ** 0.8
-    g = tn * om / tau                 # (t - t')/tau(t')
-    C = np.exp(-g)
-    x01 = x ** 0.1
-    R = C / (1.0 + x01)
-    gp = (om / tau) * (1.0 - 0.8 * x ** 0.8 / tau)
-    dC = -gp * C
-    with np.errstate(divide="ignore", invalid="ignore"):
-        dR = -gp * R - C * 0.1 * x01 / (tn * (1.0 + x01) ** 2)
-    C[0], R[0] = 1.0, 1.0
-    dC[0], dR[0] = -omega, -omega
-    for k, arr in enumerate((C, dC, R, dR)):
-        rng = np.random.Generator(np.random.PCG64(seed + k))
-        xi = rng.uniform(-1.0, 1.0, size=(N, L))
-        hist[:, :, k] = arr * (1.0 + jitter * xi)
+    rngs = [np.random.Generator(np.random.PCG64(seed + k)) for k in range(4)]
+    # row blocks bound the temporaries (nine N x L arrays otherwise: 77 GB at L = N = 32768); the
+    # jitter streams are consumed row-major, so the blocking does not change which number goes where
+    blk = N if N * L <= (1 << 27) else max(1, (1 << 27) // L)
+    for r0 in range(0, N, blk):
+        r1 = min(N, r0 + blk)
+        tn = t[r0:r1, None]
+        th = theta[None, :]
+        om = omega[None, :]
+        x = th * tn                       # t' = theta t
+        tau = 1.0 + x ** 0.8
+        g = tn * om / tau                 # (t - t')/tau(t')
+        C = np.exp(-g)
+        x01 = x ** 0.1
+        R = C / (1.0 + x01)
+        gp = (om / tau) * (1.0 - 0.8 * x ** 0.8 / tau)
+        dC = -gp * C
+        with np.errstate(divide="ignore", invalid="ignore"):
+            dR = -gp * R - C * 0.1 * x01 / (tn * (1.0 + x01) ** 2)
+        if r0 == 0:
+            C[0], R[0] = 1.0, 1.0
+            dC[0], dR[0] = -omega, -omega
+        for k, arr in enumerate((C, dC, R, dR)):
+            xi = rngs[k].uniform(-1.0, 1.0, size=(r1 - r0, L))
+            hist[r0:r1, :, k] = arr * (1.0 + jitter * xi)
     return t, mu, hist
 
 
