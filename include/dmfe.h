@@ -132,7 +132,10 @@ DMFE_API int dmfe_init_state(dmfe_ctx *ctx, dmfe_state *st, double h0);
  * fixed_step != 0: no controller, the row is always appended.  Otherwise the controller of
  * PAPER.md:320 (G20): eps_RK > 2 tol or non-finite -> drop the last 10 rows, h/2, *accepted = 0;
  * else append, h *= 0.9 if eps_RK > tol, h *= 1.01 if eps_RK < tol/2, *accepted = 1.
- * Exactly one scalar record returns to the host per call. */
+ * Exactly one scalar record (128 bytes) returns to the host per call; it is read as soon as the
+ * pre-pass of the last stage has taken the decision, so on return the evaluation that completes
+ * the appended row (its derivative, mu, E) may still be running on the context's stream: work
+ * queued on that stream is ordered behind it, other streams must synchronise with it. */
 DMFE_API int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *accepted);
 
 /* Selective history reduction, Eq.(26)-(27): drop row n if eps_sparse < tol/10,

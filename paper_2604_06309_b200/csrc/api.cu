@@ -48,6 +48,8 @@ static void free_all(dmfe_ctx *c) {
   for (int k = 0; k < 2 * c->ev_made; ++k) cudaEventDestroy(c->ev[k]);
   if (c->h_scal) cudaFreeHost(c->h_scal);
   if (c->h_iscal) cudaFreeHost(c->h_iscal);
+  if (c->side) cudaStreamDestroy(c->side);
+  if (c->ev_decided) cudaEventDestroy(c->ev_decided);
 }
 
 int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_ctx **out) {
@@ -94,6 +96,8 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
     if (e == cudaSuccess) e = cudaMalloc(&c->rk, sizeof(double) * 8 * (size_t)L);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_scal, sizeof(double) * SC_COUNT);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_iscal, sizeof(int32_t) * IS_COUNT);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_decided, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->scal, 0, sizeof(double) * SC_COUNT, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->iscal, 0, sizeof(int32_t) * IS_COUNT, c->stream);
     if (e != cudaSuccess) {

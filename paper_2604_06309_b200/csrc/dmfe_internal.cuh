@@ -80,6 +80,10 @@ struct dmfe_ctx {
   // pinned host scalars for the one-record-per-step readback
   double *h_scal;
   int32_t *h_iscal;
+  // the record is copied on a side stream as soon as the last stage's pre-pass has taken the
+  // decision, while the evaluation that completes the appended row still runs on `stream`
+  cudaStream_t side;
+  cudaEvent_t ev_decided;
 };
 
 #define CUDA_TRY(ctx, call)                              \
@@ -132,6 +136,7 @@ struct dmfe_stage {
   double *rk;          // [4][2L]: q1, q2, delta, F
   double *scal;
   int32_t *iscal;
+  cudaEvent_t after_prepass;  // optional: recorded on the stream between the pre-pass and the pair kernel
 };
 
 // tables.cu

@@ -53,6 +53,30 @@ struct RhsArgs {
   dmfe_rhs_out out;
 };
 
+// Programmatic dependent launch (both kernels of a right-hand side are launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization): a kernel lets its successor in the stream
+// start launching at once and itself waits, before it touches anything a predecessor wrote, until
+// the predecessor grid has completed and its writes are visible.  The launch latency of each of
+// the 20 kernels of an RK step is hidden behind the kernel before it.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t stream,
+                       Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(block);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 __device__ __forceinline__ double4 ld_cell(const double4 *p) {
   double4 v;
   asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
@@ -143,6 +167,40 @@ __device__ __forceinline__ int row_search(const double *__restrict__ t, int lo, 
   return lo;
 }
 
+// The same n, found from a guess g (any value): bracket by doubling steps away from g, then bisect.
+// prepare_kernel passes the value the previous evaluation left in the table: successive stages
+// differ by a fraction of a step, so the bracket closes after one or two loads instead of log2 M.
+__device__ __forceinline__ int row_search_from(const double *__restrict__ t, int top, int g, double tau) {
+  g = min(max(g, 0), top);
+  int lo, hi;
+  if (__ldg(t + g) <= tau) {
+    lo = g;
+    for (int st = 1;; st <<= 1) {
+      const int nx = min(lo + st, top);
+      if (nx == lo) return lo;  // lo == top
+      if (__ldg(t + nx) <= tau) {
+        lo = nx;
+      } else {
+        hi = nx - 1;
+        break;
+      }
+    }
+  } else {  // g >= 1 here because t[0] = 0 <= tau
+    hi = g - 1;
+    lo = 0;
+    for (int st = 1;; st <<= 1) {
+      const int nx = g - st;
+      if (nx <= 0) break;
+      if (__ldg(t + nx) <= tau) {
+        lo = nx;
+        break;
+      }
+      hi = nx - 1;
+    }
+  }
+  return row_search(t, lo, hi, tau);
+}
+
 // weights of the local interpolant in t between rows n and n+1 (PAPER.md:260 cubic Hermite);
 // quadratic (value, slope, value) when the upper row is the current row M (reading G12).  With
 // d = tau - t_n, u = d/D, v = u - 1:
@@ -193,6 +251,8 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
                                                                double2 *__restrict__ rowtab,
                                                                int32_t *__restrict__ blo, double *scal) {
   __shared__ double sm[32], se[32];
+  pdl_launch_dependents();
+  pdl_wait();
   const int k = sg.k;
   // time of the row being evaluated.  The step size of stage 0 is the controller's proposal
   // (SC_HNEXT); block 0 latches it into SC_H, which stages 1..9 read.
@@ -214,107 +274,109 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
         rowtab[e] = make_double2(tn, 1.0 / (tn1 - tn));
       } else {
         const int c = e - M;
-        blo[c] = row_search(t, 0, M - 1, __dmul_rn(theta[c], tM));
+        blo[c] = row_search_from(t, M - 1, blo[c], __dmul_rn(theta[c], tM));
       }
     }
     if (blockIdx.x > 0) return;
   }
-  if (k >= 0) {
-    // ---- stage update: rk = [4][2L]: q1, q2, delta, F ----
-    const int n2 = 2 * L, N = sg.N;
-    double *q1 = sg.rk, *q2 = sg.rk + n2, *dl = sg.rk + 2 * n2;
-    const double *F = sg.rk + 3 * n2;
-    const double hb = __dmul_rn(h, c_b_minus_bhat[k]);
-    const double h6 = h / 6.0;
-    double eacc = 0.0;
-    for (int e = threadIdx.x; e < n2; e += blockDim.x) {
-      const int l = e >> 1, comp = e & 1;
-      const size_t cellN = ((size_t)N * L + l) * 4, cellM = ((size_t)M * L + l) * 4;
-      double a, b, d, Fk;
+  // ---- block 0: optional stage update, then pack row M and reduce mu, E; a thread owns the two
+  // state entries {C, R} of a node l and keeps them in registers from the update to the sums ----
+  const int N = sg.N;
+  double2 *q1 = reinterpret_cast<double2 *>(sg.rk), *q2 = q1 + L, *dl = q2 + L;
+  const double2 *F = dl + L;  // rk = [4][L]{C,R}: q1, q2, delta, F
+  const double hb = (k >= 0) ? __dmul_rn(h, c_b_minus_bhat[k]) : 0.0;
+  const double h6 = h / 6.0;
+  double4 *rowM = const_cast<double4 *>(hist) + (size_t)M * (size_t)L;
+  double eacc = 0.0, am = 0.0, ae = 0.0;
+  __shared__ double s_c0;
+  for (int l = threadIdx.x; l < L; l += blockDim.x) {
+    double2 y;  // {C, R} of row M at node l
+    if (k >= 0) {
+      double2 a, b, d, Fk;
       if (k == 0) {
-        a = b = sg.hist[cellN + 2 * comp];
-        d = 0.0;
-        Fk = sg.hist[cellN + 2 * comp + 1];
+        const double4 c = hist[(size_t)N * (size_t)L + l];
+        a = b = make_double2(c.x, c.z);
+        d = make_double2(0.0, 0.0);
+        Fk = make_double2(c.y, c.w);
       } else {
-        a = q1[e];
-        b = q2[e];
-        d = dl[e];
-        Fk = F[e];
+        a = q1[l];
+        b = q2[l];
+        d = dl[l];
+        Fk = F[l];
       }
-      d = __dadd_rn(d, __dmul_rn(hb, Fk));
-      if (k < 9) {
-        a = __dadd_rn(a, __dmul_rn(h6, Fk));
-        if (k == 4) {
-          b = __dadd_rn(b / 25.0, __dmul_rn(9.0 / 25.0, a));
-          a = __dsub_rn(__dmul_rn(15.0, b), __dmul_rn(5.0, a));
-        }
-      } else {
-        a = __dadd_rn(__dadd_rn(b, __dmul_rn(0.6, a)), __dmul_rn(__dmul_rn(0.1, h), Fk));
-        eacc += fabs(d);
-      }
-      q1[e] = a;
-      q2[e] = b;
-      dl[e] = d;
-      sg.hist[cellM + 2 * comp] = a;  // stage state = value slots of the current row M
-    }
-    if (threadIdx.x == 0) {
-      sg.t[M] = tM;
-      if (k == 0) scal[SC_H] = h;
-    }
-    if (k == 9) {
-      // eps_RK = sum_i |delta C_i| + |delta R_i| (Eq.(25)) and the controller (PAPER.md:320, G20)
-      for (int o = 16; o > 0; o >>= 1) eacc += __shfl_xor_sync(0xffffffffu, eacc, o);
-      if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = eacc;
-      __syncthreads();
-      if (threadIdx.x == 0) {
-        double eps = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) eps += sm[w];
-        double hn = h;
-        int accept = 1;
-        if (!sg.fixed_step) {
-          if (!isfinite(eps) || eps > 2.0 * sg.tol) {
-            accept = 0;
-            hn = fmin(h / 2.0, sg.cap);
-          } else {
-            if (eps > sg.tol)
-              hn = 0.9 * h;
-            else if (eps < sg.tol / 2.0)
-              hn = 1.01 * h;
-            hn = fmin(hn, sg.cap);
+      auto upd = [&](double &av, double &bv, double &dv, double Fv) {
+        dv = __dadd_rn(dv, __dmul_rn(hb, Fv));
+        if (k < 9) {
+          av = __dadd_rn(av, __dmul_rn(h6, Fv));
+          if (k == 4) {
+            bv = __dadd_rn(bv / 25.0, __dmul_rn(9.0 / 25.0, av));
+            av = __dsub_rn(__dmul_rn(15.0, bv), __dmul_rn(5.0, av));
           }
+        } else {
+          av = __dadd_rn(__dadd_rn(bv, __dmul_rn(0.6, av)), __dmul_rn(__dmul_rn(0.1, h), Fv));
+          eacc += fabs(dv);
         }
-        scal[SC_EPS] = eps;
-        scal[SC_HNEXT] = hn;
-        scal[SC_ACCEPT] = (double)accept;
-        sg.iscal[IS_ACCEPT] = accept;
-      }
+      };
+      upd(a.x, b.x, d.x, Fk.x);
+      upd(a.y, b.y, d.y, Fk.y);
+      q1[l] = a;
+      q2[l] = b;
+      dl[l] = d;
+      double *cell = reinterpret_cast<double *>(rowM + l);
+      cell[0] = a.x;  // stage state = value slots of the current row M
+      cell[2] = a.y;
+      y = a;
+    } else {
+      const double4 c = rowM[l];
+      y = make_double2(c.x, c.z);
     }
-    __syncthreads();  // the row written above is read below by other threads of this block
+    cur[l] = y;
+    if (l == 0) s_c0 = y.x;
+    const double fp = horner(mc.c1, mc.pmax - 1, y.x), fpp = horner(mc.c2, mc.pmax - 2, y.x);
+    const double nj = nu[l];
+    am += nj * (fpp * y.y * y.x + fp * y.y);
+    ae += nj * (fp * y.y);
   }
-  const double4 *row = hist + (size_t)M * (size_t)L;
-  double am = 0.0, ae = 0.0;
-  for (int j = threadIdx.x; j < L; j += blockDim.x) {
-    const double4 c = row[j];  // plain load: the value slots may have been written by this block
-    cur[j] = make_double2(c.x, c.z);
-    const double fp = horner(mc.c1, mc.pmax - 1, c.x), fpp = horner(mc.c2, mc.pmax - 2, c.x);
-    const double nj = nu[j];
-    am += nj * (fpp * c.z * c.x + fp * c.z);
-    ae += nj * (fp * c.z);
+  if (k >= 0 && threadIdx.x == 0) {
+    sg.t[M] = tM;
+    if (k == 0) scal[SC_H] = h;
   }
   for (int o = 16; o > 0; o >>= 1) {
     am += __shfl_xor_sync(0xffffffffu, am, o);
     ae += __shfl_xor_sync(0xffffffffu, ae, o);
+    eacc += __shfl_xor_sync(0xffffffffu, eacc, o);
   }
   const int w = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  __syncthreads();  // sm[] may still be read by thread 0 (stage 9)
-  if ((threadIdx.x & 31) == 0) sm[w] = am, se[w] = ae;
+  __shared__ double sx[32];
+  if ((threadIdx.x & 31) == 0) sm[w] = am, se[w] = ae, sx[w] = eacc;
   __syncthreads();
   if (threadIdx.x == 0) {
-    double tm = 0.0, te = 0.0;
-    for (int q = 0; q < nw; ++q) tm += sm[q], te += se[q];
-    const double c0 = row[0].x;
+    double tm = 0.0, te = 0.0, eps = 0.0;
+    for (int q = 0; q < nw; ++q) tm += sm[q], te += se[q], eps += sx[q];
+    const double c0 = s_c0;
     scal[SC_MU] = mc.T + tM * tm + mc.beta0 * horner(mc.c1, mc.pmax - 1, c0) * c0;
     scal[SC_E] = -tM * te - mc.beta0 * horner(mc.c0, mc.pmax, c0);
+    if (k == 9) {
+      // eps_RK = sum_i |delta C_i| + |delta R_i| (Eq.(25)) and the controller (PAPER.md:320, G20)
+      double hn = h;
+      int accept = 1;
+      if (!sg.fixed_step) {
+        if (!isfinite(eps) || eps > 2.0 * sg.tol) {
+          accept = 0;
+          hn = fmin(h / 2.0, sg.cap);
+        } else {
+          if (eps > sg.tol)
+            hn = 0.9 * h;
+          else if (eps < sg.tol / 2.0)
+            hn = 1.01 * h;
+          hn = fmin(hn, sg.cap);
+        }
+      }
+      scal[SC_EPS] = eps;
+      scal[SC_HNEXT] = hn;
+      scal[SC_ACCEPT] = (double)accept;
+      sg.iscal[IS_ACCEPT] = accept;
+    }
   }
 }
 
@@ -370,6 +432,8 @@ template <int S, int PD, int SM>
 __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
   constexpr bool SMT = SM >= 1, SMR = SM == 2;
   extern __shared__ double4 smem_dyn[];
+  pdl_launch_dependents();
+  pdl_wait();
   const int L = a.L, M = a.M;
   const double2 *cur = a.cur;
   const double2 *rowtab = a.rowtab;
@@ -643,9 +707,9 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
     memset(&sg, 0, sizeof(sg));
     sg.k = -1;
   }
-  prepare_kernel<<<pb, PREP_THREADS, 0, ctx->stream>>>(L, M, ctx->model, sg, ctx->theta, ctx->nu, t,
-                                                       (const double4 *)hist, ctx->cur, ctx->rowtab, ctx->blo,
-                                                       ctx->scal);
+  CUDA_TRY(ctx, launch_pdl(prepare_kernel, pb, PREP_THREADS, 0, ctx->stream, L, M, ctx->model, sg, ctx->theta,
+                           ctx->nu, t, (const double4 *)hist, ctx->cur, ctx->rowtab, ctx->blo, ctx->scal));
+  if (stage && stage->after_prepass) CUDA_TRY(ctx, cudaEventRecord(stage->after_prepass, ctx->stream));
   RhsArgs a;
   a.L = L;
   a.M = M;
@@ -708,7 +772,7 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
     auto kfn = history_integrals_kernel<S_, PD_, SM_>;                                                  \
     if (smem + 4096 > 48 * 1024)                                                                        \
       CUDA_TRY(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-    kfn<<<grid, RHS_THREADS, smem, ctx->stream>>>(a, ctx->model);                                       \
+    CUDA_TRY(ctx, launch_pdl(kfn, grid, RHS_THREADS, smem, ctx->stream, a, ctx->model));                \
   } while (0)
 #define DMFE_LAUNCH(S_, PD_)       \
   do {                             \

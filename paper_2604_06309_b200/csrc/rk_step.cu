@@ -63,7 +63,6 @@ int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *acc
   if (st->n_rows + 1 > st->n_cap) return DMFE_ECAPACITY;
   const int L = ctx->p.L;
   const int N = st->n_rows - 1, M = N + 1;
-  cudaStream_t s = ctx->stream;
   double *F = ctx->rk + 6 * (size_t)L;
   dmfe_stage sg;
   sg.N = N;
@@ -86,13 +85,19 @@ int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *acc
       deriv_row = st->hist + (size_t)M * (size_t)L * 4;
     }
     sg.k = k;
+    sg.after_prepass = (k == 9) ? ctx->ev_decided : nullptr;
     const int rc = dmfe_launch_rhs(ctx, M, st->n_cap, st->t, st->mu, st->hist, &o, &sg, deriv_row);
     if (rc != DMFE_OK) return rc;
     st->n_rhs++;
   }
   // the one record that returns to the host: {accept flag, eps_RK, next h}
-  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->scal, sizeof(double) * SC_COUNT, cudaMemcpyDeviceToHost, s));
-  CUDA_TRY(ctx, cudaStreamSynchronize(s));
+  // It is final once the pre-pass of the last stage has run, so it is copied on the side stream
+  // behind that point: the host learns the decision and queues the next step while the evaluation
+  // that completes the appended row is still running.
+  CUDA_TRY(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_decided, 0));
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->h_scal, ctx->scal, sizeof(double) * SC_COUNT, cudaMemcpyDeviceToHost,
+                                ctx->side));
+  CUDA_TRY(ctx, cudaStreamSynchronize(ctx->side));
   const int acc = ctx->h_scal[SC_ACCEPT] != 0.0;
   st->eps_rk = ctx->h_scal[SC_EPS];
   st->h = ctx->h_scal[SC_HNEXT];

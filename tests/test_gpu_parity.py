@@ -156,18 +156,16 @@ def test_rhs_matches_oracle_synthetic(D, L, lo, hi, t_max, lam):
     compare_rhs(g, ref)
 
 
-def test_rhs_full_bench_size_sampled_targets(D):
-    """BASELINE.json config 2 at its full size (L = N = 4096, the launch configuration bench.py
-    times): every output of seeded blocks of targets against the oracle run on those targets."""
-    import torch
-    L, s, t_max, lam = 4096, 4, 1e4, [0, 0, 0, 1.0]
+def _sampled_blocks_parity(D, L, s, t_max, lam, lo, hi, n_blocks):
+    """Every output of seeded blocks of 32 targets (first and last block included) of one full-size
+    evaluation against the oracle run on those targets with the library's tables."""
     ctx = D.dmfe_create(L, s, t_max, lam, T=0.5)
     try:
         tab = D.dmfe_get_tables(ctx, L, want_pairs=False)
-        t, mu, hist = inputs.synthetic_history(tab["theta"], tab["omega"], L, -2.0, 4.0)
+        t, mu, hist = inputs.synthetic_history(tab["theta"], tab["omega"], L, lo, hi)
         g = gpu_rhs(D, ctx, L, t, mu, hist, L, want_rows=False)
-        rng = np.random.Generator(np.random.PCG64(4096))
-        blocks = np.sort(rng.choice(L // 32, size=8, replace=False)) * 32
+        rng = np.random.Generator(np.random.PCG64(L))
+        blocks = np.sort(rng.choice(L // 32, size=n_blocks, replace=False)) * 32
         blocks = np.unique(np.concatenate([[0], blocks, [L - 32]]))
         grid = _oracle_grid_from_library(tab, L, s, t_max)
         model = O.Model(np.array(lam, dtype=np.float64), 0.5, 0.0)
@@ -183,8 +181,22 @@ def test_rhs_full_bench_size_sampled_targets(D):
                 e = np.abs(g[name][targets] - ref["deriv"][:, k])
                 assert np.max(e / (RTOL * ref["scale"][:, k] + 1e-300)) <= 1.0, name
         assert abs(g["mu_out"][0] - ref["mu"]) <= RTOL * abs(ref["mu"])
+        assert abs(g["energy"][0] - ref["E"]) <= RTOL * max(abs(ref["E"]), 1e-300)
     finally:
         D.dmfe_destroy(ctx)
+
+
+def test_rhs_full_bench_size_sampled_targets(D):
+    """BASELINE.json config 2 at its full size (L = N = 4096, the launch configuration bench.py
+    times)."""
+    _sampled_blocks_parity(D, 4096, 4, 1e4, [0, 0, 0, 1.0], -2.0, 4.0, n_blocks=8)
+
+
+def test_rhs_large_grid_global_table_path_sampled_targets(D):
+    """Config-5 recipe (mixed f, rows on [1e-2, 1e7]) at L = N = 10240: above L = 9685 the per-call
+    tables (24 L bytes) no longer fit in shared memory and the kernel reads them from global
+    memory -- the launch configuration of the L = 16384 and 32768 points of the scaling sweep."""
+    _sampled_blocks_parity(D, 10240, 4, 1e7, [0, 0, 1.0, 0.8, 0.5], -2.0, 7.0, n_blocks=6)
 
 
 def test_rhs_rows_in_a_larger_buffer(D):
