@@ -199,6 +199,46 @@ def test_rhs_large_grid_global_table_path_sampled_targets(D):
     _sampled_blocks_parity(D, 10240, 4, 1e7, [0, 0, 1.0, 0.8, 0.5], -2.0, 7.0, n_blocks=6)
 
 
+def test_rhs_mode1_row_table_in_global_memory_sampled_targets(D):
+    """Config-5 recipe at L = N = 8192: the current row and the brackets fit in shared memory, the
+    row table does not (third launch configuration of the pair kernel, the one of the L = 8192
+    point of the scaling sweep)."""
+    _sampled_blocks_parity(D, 8192, 4, 1e7, [0, 0, 1.0, 0.8, 0.5], -2.0, 7.0, n_blocks=4)
+
+
+def test_rhs_closed_form_constant_history_full_size_all_targets(D):
+    """A property that holds at any size, checked on every target of the bench-size evaluation
+    (L = N = 4096, log-spaced rows of config 2) without the oracle: for the constant history
+    C = R = 1 (slopes 0), f = q^2/2 and mu_n = T + 2 t_n every interpolation is exact and the sums
+    need only sum(nu) = 1 (oracle pin P4, Eq.(1), (13), (14)):
+      mu = T + 2t, E = -t, d1C_i = -T - t w_i, d1R_i = -(T + 2t) + t w_i,
+      d2C_i = T + t w_i, d2R_i = T + 2 theta_i t - t w_i, F = d1 + theta_i d2      (w_i = 1 - theta_i)."""
+    L, s, t_max, T = 4096, 4, 1e4, 0.7
+    ctx = D.dmfe_create(L, s, t_max, [0.0, 0.0, 1.0], T=T)
+    try:
+        tab = D.dmfe_get_tables(ctx, L, want_pairs=False)
+        th, om = tab["theta"], tab["omega"]
+        t = inputs.log_times(L, -2.0, 4.0)
+        mu = T + 2.0 * t
+        hist = np.zeros((L, L, 4))
+        hist[:, :, 0] = 1.0
+        hist[:, :, 2] = 1.0
+        g = gpu_rhs(D, ctx, L, t, mu, hist, L, want_rows=False)
+    finally:
+        D.dmfe_destroy(ctx)
+    tM = t[-1]
+    tol = 1e-12 * (1.0 + tM)
+    assert abs(g["mu_out"][0] - (T + 2 * tM)) < tol and abs(g["energy"][0] + tM) < tol
+    assert np.abs(g["sums"] - 1.0).max() < 1e-12                      # all eight sums are sum(nu) = 1
+    assert np.abs(g["d1C"] - (-T - tM * om)).max() < tol
+    assert np.abs(g["d1R"] - (-(T + 2 * tM) + tM * om)).max() < tol
+    assert np.abs(g["d2C"] - (T + tM * om)).max() < tol
+    assert np.abs(g["d2R"] - (T + 2 * th * tM - tM * om)).max() < tol
+    FC = (-T - tM * om) + th * (T + tM * om)
+    FR = (-(T + 2 * tM) + tM * om) + th * (T + 2 * th * tM - tM * om)
+    assert np.abs(g["F"][:, 0] - FC).max() < tol and np.abs(g["F"][:, 1] - FR).max() < tol
+
+
 def test_rhs_rows_in_a_larger_buffer(D):
     """n_rows < n_cap: rows beyond the current one are never touched (filled with NaN here)."""
     L, N, s = 80, 20, 4
