@@ -341,6 +341,97 @@ def complete_row(H: History):
     H.n_rows = M + 1
 
 
+# ---- Dormand-Prince 5(4) ("uses the Dormand-Prince method [63] at short times"),
+# the textbook tableau of ref. [63]; row 7 of A equals the fifth-order weights b (FSAL)
+DP_C = np.array([0.0, 1.0 / 5.0, 3.0 / 10.0, 4.0 / 5.0, 8.0 / 9.0, 1.0, 1.0])
+DP_A = np.zeros((7, 7))
+DP_A[1, :1] = [1.0 / 5.0]
+DP_A[2, :2] = [3.0 / 40.0, 9.0 / 40.0]
+DP_A[3, :3] = [44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0]
+DP_A[4, :4] = [19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0]
+DP_A[5, :5] = [9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0]
+DP_A[6, :6] = [35.0 / 384.0, 0.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0]
+DP_B = DP_A[6].copy()
+DP_BHAT = np.array([5179.0 / 57600.0, 0.0, 7571.0 / 16695.0, 393.0 / 640.0, -92097.0 / 339200.0,
+                    187.0 / 2100.0, 1.0 / 40.0])
+DP_SWITCH = 3.3  # switch to SSPRK(10,4) when h 4 sqrt(f''(1)) reaches the real-axis limit of DP5 (3.3066; G21)
+
+
+def dopri54(F, y, t0: float, h: float, F1):
+    """One Dormand-Prince 5(4) step for y' = F(t, y).  F1 = F(t0, y) (stored with the history).
+    Stage i: y_i = y + h sum_{j<i} a_ij k_j (terms in the order j = 1, 2, ...; zero coefficients
+    skipped), k_i = F(t0 + c_i h, y_i); y_next = y_7; k_7 = F(t0 + h, y_next) is the derivative of
+    the new point (FSAL) and enters the error estimate delta = h sum_j (b_j - bhat_j) k_j.
+    Returns (y_next, k_7, delta)."""
+    k = [F1]
+    yi = y
+    for i in range(1, 7):
+        acc = None
+        for j in range(i):
+            if DP_A[i, j] == 0.0:
+                continue
+            term = DP_A[i, j] * k[j]
+            acc = term if acc is None else acc + term
+        yi = y + h * acc
+        k.append(F(t0 + DP_C[i] * h, yi))
+    acc = None
+    for j in range(7):
+        e = DP_B[j] - DP_BHAT[j]
+        if e == 0.0:
+            continue
+        term = e * k[j]
+        acc = term if acc is None else acc + term
+    return yi, k[6], h * acc
+
+
+def dp_step(H: "History", h: float):
+    """One Dormand-Prince step from the last complete row N: writes row N+1 (values, then its
+    derivative, mu and E from the FSAL evaluation) and returns eps_RK of Eq.(25).  Does not accept
+    the row (n_rows unchanged)."""
+    N = H.n_rows - 1
+    M = N + 1
+    assert M < H.n_cap
+    L = H.grid.L
+    y = np.concatenate([H.hist[N, :, 0], H.hist[N, :, 2]])
+    F1 = np.concatenate([H.hist[N, :, 1], H.hist[N, :, 3]])
+    last = {}
+
+    def F(ts, q):
+        H.t[M] = ts
+        H.hist[M, :, 0], H.hist[M, :, 2] = q[:L], q[L:]
+        H.hist[M, :, 1], H.hist[M, :, 3] = 0.0, 0.0
+        FC, FR, mu, E = H.rhs_current(M)
+        last["mu"], last["E"] = mu, E
+        return np.concatenate([FC, FR])
+
+    ynew, k7, delta = dopri54(F, y, H.t[N], h, F1)
+    H.hist[M, :, 1], H.hist[M, :, 3] = k7[:L], k7[L:]
+    H.mu[M], H.E[M] = last["mu"], last["E"]
+    return float(np.sum(np.abs(delta)))
+
+
+def dp_controller_step(H: "History", h: float, tol: float):
+    """One adaptive Dormand-Prince step with the controller of PAPER.md:320 (reading G20); no step
+    cap here: the caller switches to SSPRK(10,4) when h reaches the stability boundary (G21).
+    Returns (accepted, h_next, eps_RK)."""
+    eps = dp_step(H, h)
+    if not np.isfinite(eps) or eps > 2.0 * tol:
+        H.n_rows = max(1, H.n_rows - 10)
+        return False, h / 2.0, eps
+    H.n_rows += 1
+    if eps > tol:
+        h = 0.9 * h
+    elif eps < tol / 2.0:
+        h = 1.01 * h
+    return True, h, eps
+
+
+def dp_must_switch(model: "Model", h: float) -> bool:
+    """Dormand-Prince "until the time step grows sufficiently to reach the boundary of
+    its stability domain"; with the spectral bound 4 sqrt(f''(1)) of Eq.(24) (reading G21)."""
+    return h * 4.0 * np.sqrt(model.f(1.0, 2)) >= DP_SWITCH
+
+
 def h_stab(model: Model) -> float:
     """Step cap from Eq.(24) and the real-axis stability limit of SSPRK(10,4)."""
     return STAB_REAL_AXIS / (4.0 * np.sqrt(model.f(1.0, 2)))
@@ -400,10 +491,12 @@ def sparsify(H: History, tol: float, protect_last: int = 12):
 
 
 def run_adaptive(grid: Grid, model: Model, t_end: float, tol: float, h0=1e-3, n_cap=2048,
-                 sp_every=200, protect_last=12, h_min=1e-12, max_steps=10 ** 9, log=None):
-    """Adaptive trajectory with periodic sparsification."""
+                 sp_every=200, protect_last=12, h_min=1e-12, max_steps=10 ** 9, log=None, startup="ssprk"):
+    """Adaptive trajectory with periodic sparsification.
+    startup = "dp": Dormand-Prince steps until dp_must_switch, then h/2 and SSPRK(10,4)."""
     H = History(grid, model, n_cap)
     h = min(h0, h_stab(model))
+    use_dp = startup == "dp"
     acc = 0
     steps = 0
     while H.t[H.n_rows - 1] < t_end and steps < max_steps:
@@ -413,7 +506,10 @@ def run_adaptive(grid: Grid, model: Model, t_end: float, tol: float, h0=1e-3, n_
             if H.n_rows + 1 >= n_cap:
                 raise RuntimeError("capacity: sparsify freed nothing (%d rows)" % before)
             acc += 1 if acc % sp_every == 0 else 0
-        ok, h, eps = controller_step(H, h, tol)
+        if use_dp and dp_must_switch(model, h):
+            use_dp = False
+            h = min(h / 2.0, h_stab(model))
+        ok, h, eps = dp_controller_step(H, h, tol) if use_dp else controller_step(H, h, tol)
         steps += 1
         if ok:
             acc += 1
