@@ -138,6 +138,19 @@ DMFE_API int dmfe_init_state(dmfe_ctx *ctx, dmfe_state *st, double h0);
  * queued on that stream is ordered behind it, other streams must synchronise with it. */
 DMFE_API int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *accepted);
 
+/* One Dormand-Prince 5(4) step (the start-up integrator "at short times", textbook
+ * tableau of ref. [63]) from the last row, all stages on the device; same state, same record and
+ * same controller as dmfe_rk_step except that no step cap is applied: the caller switches to
+ * dmfe_rk_step when h 4 sqrt(f''(1)) reaches the stability boundary of the method (3.3; reading
+ * G21 in DESIGN.md) with dmfe_set_step_size(h/2).  Six evaluations per step; the
+ * last one (FSAL) stores the derivative, mu and E of the appended row and enters the error
+ * estimate, so the record is read after it.  Synchronises on the context's stream. */
+DMFE_API int dmfe_dp_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *accepted);
+
+/* Sets the step size the next dmfe_rk_step / dmfe_dp_step starts from (device copy and st->h).
+ * h <= 0: DMFE_EINVAL.  Asynchronous. */
+DMFE_API int dmfe_set_step_size(dmfe_ctx *ctx, dmfe_state *st, double h);
+
 /* Selective history reduction, Eq.(26)-(27): drop row n if eps_sparse < tol/10,
  * then skip to n+2; row 0 and the last protect_last rows are kept; t, mu, energy and the packed
  * rows are compacted on the device.  keep_mask: optional HOST [n_rows before] bytes (test hook). */

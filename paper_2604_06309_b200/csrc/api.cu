@@ -37,6 +37,7 @@ static void free_all(dmfe_ctx *c) {
   cudaFree(c->scal);
   cudaFree(c->iscal);
   cudaFree(c->rk);
+  cudaFree(c->dpk);
   cudaFree(c->eps_sp);
   cudaFree(c->keep);
   cudaFree(c->newidx);

@@ -63,6 +63,7 @@ struct dmfe_ctx {
   double *scal;     // [SC_COUNT]
   int32_t *iscal;   // [IS_COUNT]
   double *rk;       // [4][L][2]: q1, q2, delta, F
+  double *dpk;      // [7][L][2]: Dormand-Prince k_1..k_6 and F (allocated by the first dmfe_dp_step)
   double *eps_sp;   // [n] sparsify residuals (grown on demand)
   int32_t *keep;    // [n] keep flags / scan
   int32_t *newidx;  // [n] compacted source index

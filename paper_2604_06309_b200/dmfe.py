@@ -20,6 +20,7 @@ DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE
 
 EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror", "dmfe_get_tables",
            "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_init_state", "dmfe_rk_step",
+           "dmfe_dp_step", "dmfe_set_step_size",
            "dmfe_sparsify", "dmfe_set_sparsify_threshold", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
            "dmfe_probe_fp64_tflops", "dmfe_probe_load_path"]
 
@@ -80,6 +81,10 @@ def load_library():
     lib.dmfe_init_state.argtypes = [c_void_p, POINTER(dmfe_state), c_double]
     lib.dmfe_rk_step.restype = c_int
     lib.dmfe_rk_step.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32)]
+    lib.dmfe_dp_step.restype = c_int
+    lib.dmfe_dp_step.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32)]
+    lib.dmfe_set_step_size.restype = c_int
+    lib.dmfe_set_step_size.argtypes = [c_void_p, POINTER(dmfe_state), c_double]
     lib.dmfe_sparsify.restype = c_int
     lib.dmfe_sparsify.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32), c_void_p]
     lib.dmfe_set_sparsify_threshold.restype = c_int
@@ -199,6 +204,17 @@ def dmfe_rk_step(ctx, st, fixed_step=False):
     acc = c_int32(0)
     _check(load_library().dmfe_rk_step(ctx, byref(st), 1 if fixed_step else 0, byref(acc)), "dmfe_rk_step", ctx)
     return bool(acc.value)
+
+
+def dmfe_dp_step(ctx, st, fixed_step=False):
+    """Dormand-Prince 5(4) start-up step -> accepted (bool)."""
+    acc = c_int32(0)
+    _check(load_library().dmfe_dp_step(ctx, byref(st), 1 if fixed_step else 0, byref(acc)), "dmfe_dp_step", ctx)
+    return bool(acc.value)
+
+
+def dmfe_set_step_size(ctx, st, h):
+    _check(load_library().dmfe_set_step_size(ctx, byref(st), float(h)), "dmfe_set_step_size", ctx)
 
 
 def dmfe_sparsify(ctx, st, protect_last=12, want_mask=False):

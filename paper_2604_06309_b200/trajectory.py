@@ -17,6 +17,8 @@ import numpy as np
 
 from . import dmfe as D
 
+DP_SWITCH = 3.3      # real-axis stability boundary of Dormand-Prince 5(4) is 3.3066 (reading G21)
+SSPRK_STAB = 13.9    # step cap of Eq.(24) as the library applies it (include/dmfe.h)
 CONFIGS = {
     # BASELINE.json configs[2], [3] (sizes: DESIGN.md section 4)
     3: dict(lam=[0.0, 0.0, 1.0, 0.0, 0.5], T=0.5, tol=1e-8, n_cap=2048, t_max=1e5, L=512, s=4),
@@ -36,9 +38,11 @@ def observe(theta, t, row, t_w):
 
 
 def run(L, s, t_max, lam, T, tol, n_cap, t_end, h0=1e-3, sp_every=200, protect_last=12, beta0=0.0,
-        t_w=(1e2, 1e3, 1e4, 1e5), n_obs=64, max_steps=None, max_seconds=None, progress=None):
+        t_w=(1e2, 1e3, 1e4, 1e5), n_obs=64, max_steps=None, max_seconds=None, progress=None, startup="ssprk"):
     """Integrate from t = 0 to t_end.  Returns a dict with the observation records, the wall-clock
-    time at which each decade of t was first passed, and step statistics."""
+    time at which each decade of t was first passed, and step statistics.  startup = "dp": the
+    run starts with Dormand-Prince steps and switches to SSPRK(10,4) with half the step when
+    h 4 sqrt(f''(1)) reaches 3.3 (reading G21)."""
     import torch
 
     ctx = D.dmfe_create(L, s, t_max, lam, T=T, beta0=beta0, tol=tol)
@@ -50,6 +54,12 @@ def run(L, s, t_max, lam, T, tol, n_cap, t_end, h0=1e-3, sp_every=200, protect_l
         theta = D.dmfe_get_tables(ctx, L, want_pairs=False)["theta"]
         st, ten = D.make_state(L, n_cap)
         D.dmfe_init_state(ctx, st, h0)
+        lam_a = np.asarray(lam, dtype=np.float64)
+        f2_1 = 0.5 * sum(p * (p - 1) * lam_a[p] for p in range(2, len(lam_a)))       # f''(1)
+        h_switch = DP_SWITCH / (4.0 * np.sqrt(f2_1)) if f2_1 > 0 else np.inf
+        h_cap = SSPRK_STAB / (4.0 * np.sqrt(f2_1)) if f2_1 > 0 else np.inf        # Eq.(24), as dmfe_rk_step caps
+        use_dp = startup == "dp"
+        stats["dp_steps"] = 0
         # observation times: log-spaced, a record is taken at the first accepted step beyond each
         obs_times = list(np.geomspace(max(10 * h0, 1e-2), t_end, n_obs))
         next_decade = 1.0
@@ -81,9 +91,16 @@ def run(L, s, t_max, lam, T, tol, n_cap, t_end, h0=1e-3, sp_every=200, protect_l
                 if forced and n_after + 2 > n_cap:
                     stats["status"] = "capacity"      # DMFE_ECAPACITY: forced passes freed nothing
                     break
+            if use_dp and st.h >= h_switch:
+                use_dp = False
+                D.dmfe_set_step_size(ctx, st, min(st.h / 2.0, h_cap))
             h_used = st.h
             try:
-                ok = D.dmfe_rk_step(ctx, st)
+                if use_dp:
+                    ok = D.dmfe_dp_step(ctx, st)
+                    stats["dp_steps"] += 1
+                else:
+                    ok = D.dmfe_rk_step(ctx, st)
             except D.DmfeError as e:
                 stats["status"] = "error %d" % e.code
                 break
@@ -141,6 +158,8 @@ def main():
     ap.add_argument("--L", type=int, default=None)
     ap.add_argument("--max-seconds", type=float, default=None)
     ap.add_argument("--log", default=None, help="append one JSON line per observation record to this file")
+    ap.add_argument("--startup", default="ssprk", choices=["ssprk", "dp"],
+                    help="dp: Dormand-Prince steps until the stability boundary, then SSPRK(10,4) (PAPER.md:316)")
     args = ap.parse_args()
     cfg = dict(CONFIGS[args.config])
     if args.L:
@@ -153,7 +172,7 @@ def main():
                                         n_rows=rec["n_rows"][-1], corr=rec["corr"][-1], wall=rec["wall"][-1],
                                         steps=stats["steps"], reverted=stats["reverted"],
                                         doublings=stats["threshold_doublings"])) + "\n")
-    out = run(t_end=args.t_end, max_seconds=args.max_seconds, progress=progress, **cfg)
+    out = run(t_end=args.t_end, max_seconds=args.max_seconds, progress=progress, startup=args.startup, **cfg)
     r = out["records"]
     line = dict(config=args.config, **cfg, t_end=args.t_end, stats=out["stats"], wall_to_t=out["wall_to_t"],
                 E_last=r["E"][-1] if r["E"] else None, corr_last=r["corr"][-1] if r["corr"] else None)

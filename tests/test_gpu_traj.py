@@ -202,3 +202,83 @@ def test_trajectory_driver_with_row_cap(D):
     assert -0.95 < rec["E"][-1] < -0.6
     assert 1.0 in rec["corr"][-1] and 0.0 < rec["corr"][-1][1.0][0] < 1.0
     assert set(out["wall_to_t"]) >= {"1", "10"}
+
+
+# ------------------------------------------------------------------ Dormand-Prince start-up (8(f)-1)
+@pytest.mark.parametrize("L,s,lam,T,beta0,h,steps", [
+    (64, 4, [0, 0, 0, 1.0], 1.0, 0.0, 0.05, 30),
+    (48, 6, [0, 0, 1.0, 0, 0.5], 0.5, 0.7, 0.02, 20),
+])
+def test_dormand_prince_fixed_step_trajectory(D, L, s, lam, T, beta0, h, steps):
+    """dmfe_dp_step against the oracle's Dormand-Prince steps (pins P11-P14) on identical inputs:
+    t, mu, E and all stored rows (values and FSAL derivatives) within 1e-9."""
+    t_max = 20.0
+    ctx = D.dmfe_create(L, s, t_max, lam, T=T, beta0=beta0)
+    try:
+        grid = _oracle_grid(D, ctx, L, s, t_max)
+        st, ten = D.make_state(L, steps + 3)
+        D.dmfe_init_state(ctx, st, h)
+        for _ in range(steps):
+            assert D.dmfe_dp_step(ctx, st, fixed_step=True)
+        got = _pull(st, ten)
+        assert st.n_rows == steps + 1 and st.n_rhs == 6 * steps
+    finally:
+        D.dmfe_destroy(ctx)
+    H = O.History(grid, O.Model(np.array(lam, dtype=np.float64), T, beta0), steps + 3)
+    for _ in range(steps):
+        O.dp_step(H, h)
+        H.n_rows += 1
+    _assert_traj_close(got, H, 1e-9)
+    assert np.max(np.abs(got[3][:, -1, 0] - 1.0)) < 1e-13 and np.max(np.abs(got[3][:, -1, 2] - 1.0)) < 1e-13
+
+
+def test_dormand_prince_startup_decisions_and_switch(D):
+    """Adaptive start-up: Dormand-Prince until h 4 sqrt(f''(1)) >= 3.3, then h/2 and SSPRK(10,4)
+    (reading G21): accept / revert sequence, step sizes and the switch step equal the
+    oracle's; the trajectory agrees to 1e-9.  Loose tolerance so that the step reaches the boundary."""
+    L, s, t_max, tol = 48, 4, 50.0, 1.0
+    lam, T = [0, 0, 0, 1.0], 1.0
+    ctx = D.dmfe_create(L, s, t_max, lam, T=T, tol=tol)
+    try:
+        grid = _oracle_grid(D, ctx, L, s, t_max)
+        st, ten = D.make_state(L, 200)
+        D.dmfe_init_state(ctx, st, 0.42)
+        model = O.Model(np.array(lam, dtype=np.float64), T, 0.0)
+        H = O.History(grid, model, 200)
+        h, use_dp, switched_at = 0.42, True, None
+        for step in range(40):
+            if use_dp and O.dp_must_switch(model, h):
+                use_dp, switched_at = False, step
+                h = min(h / 2.0, O.h_stab(model))
+                D.dmfe_set_step_size(ctx, st, h)
+            if use_dp:
+                ok_ref, h, eps_ref = O.dp_controller_step(H, h, tol)
+                ok = D.dmfe_dp_step(ctx, st)
+            else:
+                ok_ref, h, eps_ref = O.controller_step(H, h, tol)
+                ok = D.dmfe_rk_step(ctx, st)
+            assert ok == ok_ref and st.n_rows == H.n_rows, "decision differs at step %d" % step
+            assert abs(st.h - h) <= 1e-15 * h
+            assert abs(st.eps_rk - eps_ref) <= 1e-6 * eps_ref + 1e-18
+        assert switched_at is not None and 3 <= switched_at < 39
+        got = _pull(st, ten)
+    finally:
+        D.dmfe_destroy(ctx)
+    _assert_traj_close(got, H, 1e-9)
+
+
+def test_trajectory_driver_with_dormand_prince_startup(D):
+    from paper_2604_06309_b200 import trajectory
+    kw = dict(L=64, s=4, t_max=200.0, lam=[0, 0, 0, 1.0], T=0.5, tol=1e-6, n_cap=400, t_end=8.0, sp_every=100,
+              n_obs=80, t_w=(1.0,))
+    a = trajectory.run(startup="dp", h0=1e-3, **kw)
+    b = trajectory.run(startup="ssprk", h0=1e-3, **kw)
+    assert a["stats"]["status"] == "ok" and a["stats"]["dp_steps"] > 0 and b["stats"]["dp_steps"] == 0
+    assert a["stats"]["C_diag_drift"] < 1e-12
+    # both integrators resolve the same solution within the tolerance of the run
+    ta, Ea = np.array(a["records"]["t"]), np.array(a["records"]["E"])
+    tb, Eb = np.array(b["records"]["t"]), np.array(b["records"]["E"])
+    assert abs(ta[-1] - tb[-1]) < 0.5 and len(ta) >= 4
+    # the records are taken at slightly different times: compare through the local slope of E(t)
+    slope = (Eb[-1] - Eb[-2]) / (tb[-1] - tb[-2])
+    assert abs(Ea[-1] - (Eb[-1] + slope * (ta[-1] - tb[-1]))) < 5e-5
