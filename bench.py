@@ -389,9 +389,10 @@ def run_ours(args):
     traffic, traffic_src = args.traffic_bytes, "--traffic-bytes"
     if traffic is None:
         try:   # dram bytes per launch of this kernel on this workload from the committed ncu capture
-            tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+            import csv
             key = "%s_L%d_s%d" % (args.workload, L, s)
-            traffic, traffic_src = tj[key]["dram_bytes_per_launch"], tj[key]["source"]
+            rows = {r["workload_key"]: r for r in csv.DictReader(open(os.path.join(ROOT, "profiles", "traffic.csv")))}
+            traffic, traffic_src = float(rows[key]["dram_bytes_per_launch"]), rows[key]["source"]
         except Exception:
             traffic, traffic_src = None, None
     roof.update({
