@@ -156,6 +156,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
     ap.add_argument("--t-end", type=float, default=1e3)
     ap.add_argument("--L", type=int, default=None)
+    ap.add_argument("--n-cap", type=int, default=None, help="row capacity (default: the config's hard cap)")
     ap.add_argument("--max-seconds", type=float, default=None)
     ap.add_argument("--log", default=None, help="append one JSON line per observation record to this file")
     ap.add_argument("--startup", default="ssprk", choices=["ssprk", "dp"],
@@ -164,6 +165,8 @@ def main():
     cfg = dict(CONFIGS[args.config])
     if args.L:
         cfg["L"] = args.L
+    if args.n_cap:
+        cfg["n_cap"] = args.n_cap
     progress = None
     if args.log:
         def progress(rec, stats):
