@@ -31,6 +31,9 @@ namespace {
 #ifndef DMFE_THREADS
 #define DMFE_THREADS 512
 #endif
+#ifndef DMFE_SPLIT
+#define DMFE_SPLIT 1  // 1: type-1 and type-2 halves of the pair loop in two loops; 0: one fused loop (v6)
+#endif
 #ifndef DMFE_PRELOAD
 #define DMFE_PRELOAD 0  // 1: all type-2 cell loads of a pair issued before the index stage of the next
 #endif
@@ -481,6 +484,168 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
     for (int k = 0; k < 8; ++k) acc[k] = 0.0;
     double b1c_first = 0.0;
 
+#if DMFE_SPLIT
+    // ---- loop fission: the type-1 half of Eq.(21) (S1, S3, S5, S6; coalesced rows n1, n1+1) runs in a
+    // loop of its own, then the type-2 half (S2, S4, S7, S8; gathers).  Each sum sees its terms in the
+    // same order as in the fused loop, so the results are bit-identical; the type-2 loop no longer
+    // carries the type-1 table entries, weights and cells, which leaves registers to request all of
+    // its 2 S cells at once. ----
+    {
+      uint64_t eA1 = 0, eB1 = 0;
+      double nuA = 0.0, nuB = 0.0;
+      double4 lo = make_double4(0, 0, 0, 0), hi = lo;
+      int j = tig;
+      if (j < L) {
+        eA1 = ld_stream(tab1 + j);
+        nuA = __ldg(&a.thnu[j].y);
+        lo = ld_cell(row1lo + j);
+        hi = ld_cell(row1hi + j);
+      }
+      if (j + TG < L) {
+        eB1 = ld_stream(tab1 + j + TG);
+        nuB = __ldg(&a.thnu[j + TG].y);
+      }
+      for (; j < L; j += TG) {
+        uint64_t eC1 = 0;
+        double nuC = 0.0;
+        double4 lon = make_double4(0, 0, 0, 0), hin = lon;
+        if (j + 2 * TG < L) {
+          eC1 = ld_stream(tab1 + j + 2 * TG);
+          nuC = __ldg(&a.thnu[j + 2 * TG].y);
+        }
+        if (j + TG < L) {
+          lon = ld_cell(row1lo + j + TG);
+          hin = ld_cell(row1hi + j + TG);
+        }
+        int a1;
+        double u1;
+        dmfe_tab_decode(eA1, &a1, &u1);
+        double w[S];
+        double C1 = 0.0, R1 = 0.0;
+        lagrange_weights<S>(u1, w);
+#pragma unroll
+        for (int l = 0; l < S; ++l) {
+          const double2 v = ld_tab<SMT>(cur + a1 + l);
+          C1 = fma(w[l], v.x, C1);
+          R1 = fma(w[l], v.y, R1);
+        }
+        if (top1) hi.y = 0.0, hi.w = 0.0;
+        const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
+        const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
+        if (j == 0) b1c_first = B1C;
+        const double nR1 = nuA * R1, nB1R = nuA * B1R;
+        acc[0] = fma(f2<PD>(mc, C1) * nR1, B1C, acc[0]);    // S1: K(t,s) C(t',s)
+        acc[2] = fma(f1<PD>(mc, C1), nB1R, acc[2]);         // S3: D(t,s) R(t',s)
+        acc[4] = fma(f2<PD>(mc, B1C) * nB1R, C1, acc[4]);   // S5: K(t',s) C(t,s)
+        acc[5] = fma(f1<PD>(mc, B1C), nR1, acc[5]);         // S6: D(t',s) R(t,s)
+        eA1 = eB1, eB1 = eC1, nuA = nuB, nuB = nuC, lo = lon, hi = hin;
+      }
+      // the four type-1 sums leave the registers before the type-2 loop starts
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        if (k == 1 || k == 3 || k >= 6) continue;
+        double v = acc[k];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[parity][warp][k] = v;
+      }
+    }
+    {
+      uint64_t eA2 = 0, eA3 = 0, eB2 = 0, eB3 = 0;
+      double2 tnA = make_double2(0.0, 0.0), tnB = tnA;
+      int n2A = 0;
+      double tau2A = 0.0;
+      int j = tig;
+      if (j < L) {
+        eA2 = ld_stream(tab2 + j);
+        eA3 = ld_stream(tab3 + j);
+        tnA = __ldg(a.thnu + j);
+      }
+      if (j + TG < L) {
+        eB2 = ld_stream(tab2 + j + TG);
+        eB3 = ld_stream(tab3 + j + TG);
+        tnB = __ldg(a.thnu + j + TG);
+      }
+      if (j < L)
+        n2A = index_stage<S, SMT, SMR>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnA.x, (int)(eA2 >> 48),
+                                       (int)(eA3 >> 48), &tau2A);
+      for (; j < L; j += TG) {
+        uint64_t eC2 = 0, eC3 = 0;
+        double2 tnC = make_double2(0.0, 0.0);
+        if (j + 2 * TG < L) {
+          eC2 = ld_stream(tab2 + j + 2 * TG);
+          eC3 = ld_stream(tab3 + j + 2 * TG);
+          tnC = __ldg(a.thnu + j + 2 * TG);
+        }
+        const int n2 = n2A;
+        const double4 *p2 = a.hist + (size_t)n2 * (size_t)L + (int)(eA3 >> 48);
+#if DMFE_PRELOAD
+        double4 x[S], y[S];
+#pragma unroll
+        for (int l = 0; l < S; ++l) {
+          x[l] = ld_cell(p2 + l);
+          y[l] = ld_cell(p2 + L + l);
+        }
+#endif
+        int n2B = 0;
+        double tau2B = 0.0;
+        if (j + TG < L)
+          n2B = index_stage<S, SMT, SMR>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnB.x, (int)(eB2 >> 48),
+                                         (int)(eB3 >> 48), &tau2B);
+        const double nj = tnA.y;
+        int a2, a3d;
+        double u2, u3;
+        dmfe_tab_decode(eA2, &a2, &u2);
+        dmfe_tab_decode(eA3, &a3d, &u3);
+        double w[S];
+        double C2 = 0.0, R2 = 0.0;
+        lagrange_weights<S>(u2, w);
+#pragma unroll
+        for (int l = 0; l < S; ++l) {
+          const double2 v = ld_tab<SMT>(cur + a2 + l);
+          C2 = fma(w[l], v.x, C2);
+          R2 = fma(w[l], v.y, R2);
+        }
+        if (a.out.rows2) a.out.rows2[(size_t)i * (size_t)L + (size_t)j] = n2;
+        const bool top2 = (n2 + 1 == M);
+        double h2[4];
+        {
+          const double2 rt = ld_tab<SMR>(rowtab + n2);
+          t_weights(rt.x, rt.y, tau2A, top2, h2);
+        }
+        lagrange_weights<S>(u3, w);
+        double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
+#pragma unroll
+        for (int l = 0; l < S; ++l) {
+#if DMFE_PRELOAD
+          const double4 xl = x[l], yl = y[l];
+#else
+          const double4 xl = ld_cell(p2 + l), yl = ld_cell(p2 + L + l);
+#endif
+          cl = fma(w[l], xl.x, cl);
+          dcl = fma(w[l], xl.y, dcl);
+          rl = fma(w[l], xl.z, rl);
+          drl = fma(w[l], xl.w, drl);
+          cu = fma(w[l], yl.x, cu);
+          dcu = fma(w[l], yl.y, dcu);
+          ru = fma(w[l], yl.z, ru);
+          dru = fma(w[l], yl.w, dru);
+        }
+        if (top2) dcu = 0.0, dru = 0.0;
+        const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
+        const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
+        const double nR2 = nj * R2;
+        const double K2 = f2<PD>(mc, C2) * nR2;
+        acc[1] = fma(K2, B2C, acc[1]);                            // S2: K(t,s) C(s,t')
+        acc[3] = fma(K2, B2R, acc[3]);                            // S4: K(t,s) R(s,t')
+        acc[6] = fma(f1<PD>(mc, B2C), nR2, acc[6]);               // S7: D(s,t') R(t,s)
+        acc[7] = fma(nR2, f2<PD>(mc, B2C) * B2R, acc[7]);         // S8: R(t,s) K(s,t')
+        eA2 = eB2, eA3 = eB3, tnA = tnB;
+        eB2 = eC2, eB3 = eC3, tnB = tnC;
+        n2A = n2B;
+        tau2A = tau2B;
+      }
+    }
+#else
     // ---- software pipeline over this thread's pairs p = j, j + TG, j + 2 TG, ... ----
     //   eA*: table entries of the pair being evaluated; n2A / tau2A: its row and time
     //   eB*, thB: table entries and theta_j of the next pair; eC*, thC: in flight for the one after
@@ -614,7 +779,19 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       n2A = n2B;
       tau2A = tau2B;
     }
+#endif
     // ---- reduction over j: shuffle within the warp, fixed order across the warps of the group ----
+#if DMFE_SPLIT
+    constexpr bool kViaRed = true;  // the type-1 sums are already in red[parity][warp]
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      if (!(k == 1 || k == 3 || k >= 6)) continue;
+      for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
+      if (lane == 0) red[parity][warp][k] = acc[k];
+    }
+    if (G > 1) group_barrier(1 + group, TG);
+#else
+    constexpr bool kViaRed = false;
 #pragma unroll
     for (int k = 0; k < 8; ++k)
       for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
@@ -625,13 +802,14 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       }
       group_barrier(1 + group, TG);  // red[parity] is reused two targets later: one barrier suffices
     }
+#endif
     if (tig != 0) continue;
 
     double Sd[8];
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
       double s = acc[k];
-      if (G > 1) {
+      if (G > 1 || kViaRed) {
         s = 0.0;
         for (int w = 0; w < G; ++w) s += red[parity][group * G + w][k];
       }
