@@ -34,8 +34,17 @@ namespace {
 #ifndef DMFE_SPLIT
 #define DMFE_SPLIT 1  // 1: type-1 and type-2 halves of the pair loop in two loops; 0: one fused loop (v6)
 #endif
+#ifndef DMFE_T1DEPTH
+#define DMFE_T1DEPTH 1  // how many pairs ahead the type-1 loop requests its two cells
+#endif
+#ifndef DMFE_SYNC1
+#define DMFE_SYNC1 0  // 1: CTA-wide barrier at the start of every round of targets
+#endif
+#ifndef DMFE_DIAG
+#define DMFE_DIAG 0  // timing diagnostics only (wrong results): 1 = type-1 loop alone, 2 = type-2 loop alone
+#endif
 #ifndef DMFE_PRELOAD
-#define DMFE_PRELOAD 0  // 1: all type-2 cell loads of a pair issued before the index stage of the next
+#define DMFE_PRELOAD 2  // type-2 cell loads issued before the index stage of the next pair: 1 = all 2 S, 2 = the S of the lower row, 0 = none
 #endif
 constexpr int RHS_THREADS = DMFE_THREADS;
 constexpr int PREP_THREADS = 1024;
@@ -464,7 +473,17 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
   const double tM = a.t[M];
   int parity = 0;
 
+#if DMFE_SYNC1
+  // the groups of a CTA take adjacent targets, whose type-1 rows mostly coincide or overlap (rows n1, n1+1 of
+  // target i and n1' in {n1, n1+1} of target i+1): starting their type-1 loops together lets one group's
+  // L1 fill serve the others
+  for (int base = blockIdx.x * ngroups; base < L; base += gridDim.x * ngroups, parity ^= 1) {
+    const int i = base + group;
+    __syncthreads();
+    if (i >= L) continue;
+#else
   for (int i = blockIdx.x * ngroups + group; i < L; i += gridDim.x * ngroups, parity ^= 1) {
+#endif
     const uint64_t *tab1 = a.tab + (size_t)i * (size_t)L, *tab2 = tab1 + plane, *tab3 = tab2 + plane;
     const double th_i = a.theta[i], om_i = a.omega[i];
     // type-1: one row search per target, tau = theta_i t  (Eq.(19)); blo[i] is exactly that row
@@ -501,13 +520,29 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         lo = ld_cell(row1lo + j);
         hi = ld_cell(row1hi + j);
       }
+#if DMFE_T1DEPTH == 2
+      double4 lon = make_double4(0, 0, 0, 0), hin = lon;
+#endif
       if (j + TG < L) {
         eB1 = ld_stream(tab1 + j + TG);
         nuB = __ldg(&a.thnu[j + TG].y);
+#if DMFE_T1DEPTH == 2
+        lon = ld_cell(row1lo + j + TG);
+        hin = ld_cell(row1hi + j + TG);
+#endif
       }
-      for (; j < L; j += TG) {
+      for (; j < L && DMFE_DIAG != 2; j += TG) {
         uint64_t eC1 = 0;
         double nuC = 0.0;
+#if DMFE_T1DEPTH == 2
+        double4 lo2 = make_double4(0, 0, 0, 0), hi2 = lo2;
+        if (j + 2 * TG < L) {
+          eC1 = ld_stream(tab1 + j + 2 * TG);
+          nuC = __ldg(&a.thnu[j + 2 * TG].y);
+          lo2 = ld_cell(row1lo + j + 2 * TG);
+          hi2 = ld_cell(row1hi + j + 2 * TG);
+        }
+#else
         double4 lon = make_double4(0, 0, 0, 0), hin = lon;
         if (j + 2 * TG < L) {
           eC1 = ld_stream(tab1 + j + 2 * TG);
@@ -517,6 +552,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
           lon = ld_cell(row1lo + j + TG);
           hin = ld_cell(row1hi + j + TG);
         }
+#endif
         int a1;
         double u1;
         dmfe_tab_decode(eA1, &a1, &u1);
@@ -539,6 +575,9 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         acc[4] = fma(f2<PD>(mc, B1C) * nB1R, C1, acc[4]);   // S5: K(t',s) C(t,s)
         acc[5] = fma(f1<PD>(mc, B1C), nR1, acc[5]);         // S6: D(t',s) R(t,s)
         eA1 = eB1, eB1 = eC1, nuA = nuB, nuB = nuC, lo = lon, hi = hin;
+#if DMFE_T1DEPTH == 2
+        lon = lo2, hin = hi2;
+#endif
       }
       // the four type-1 sums leave the registers before the type-2 loop starts
 #pragma unroll
@@ -568,7 +607,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       if (j < L)
         n2A = index_stage<S, SMT, SMR>(rowtab, blo, a.hist, L, th_i, om_i, tM, tnA.x, (int)(eA2 >> 48),
                                        (int)(eA3 >> 48), &tau2A);
-      for (; j < L; j += TG) {
+      for (; j < L && DMFE_DIAG != 1; j += TG) {
         uint64_t eC2 = 0, eC3 = 0;
         double2 tnC = make_double2(0.0, 0.0);
         if (j + 2 * TG < L) {
@@ -578,13 +617,17 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         }
         const int n2 = n2A;
         const double4 *p2 = a.hist + (size_t)n2 * (size_t)L + (int)(eA3 >> 48);
-#if DMFE_PRELOAD
+#if DMFE_PRELOAD == 1
         double4 x[S], y[S];
 #pragma unroll
         for (int l = 0; l < S; ++l) {
           x[l] = ld_cell(p2 + l);
           y[l] = ld_cell(p2 + L + l);
         }
+#elif DMFE_PRELOAD == 2  // lower row only
+        double4 x[S];
+#pragma unroll
+        for (int l = 0; l < S; ++l) x[l] = ld_cell(p2 + l);
 #endif
         int n2B = 0;
         double tau2B = 0.0;
@@ -616,8 +659,10 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
 #pragma unroll
         for (int l = 0; l < S; ++l) {
-#if DMFE_PRELOAD
+#if DMFE_PRELOAD == 1
           const double4 xl = x[l], yl = y[l];
+#elif DMFE_PRELOAD == 2
+          const double4 xl = x[l], yl = ld_cell(p2 + L + l);
 #else
           const double4 xl = ld_cell(p2 + l), yl = ld_cell(p2 + L + l);
 #endif
