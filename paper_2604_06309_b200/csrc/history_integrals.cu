@@ -23,7 +23,9 @@
 // a bisection inside the bracket [blo[l*], blo[l*+1]] of the grid cell theta_l* <= phi2 < theta_l*+1
 // that the phi2 stencil start already identifies -- same predicate and same result as a full
 // bisection.  The loop over j is software-pipelined: while pair p is evaluated, the table entries
-// of pair p+2 are in flight and the index stage of pair p+1 (bracket, bisection) has run.
+// of pair p+2 are in flight and the index stage of pair p+1 (bracket, bisection) has run.  It runs
+// twice per target (DMFE_SPLIT): the type-1 half of Eq.(21) first, then the type-2 half; every sum
+// receives its terms in the same order either way.
 #include "dmfe_internal.cuh"
 
 namespace {
