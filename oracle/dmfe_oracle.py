@@ -9,8 +9,11 @@ Pins (tests/test_oracle_*.py, all `-m "not gpu"`): P1 polynomial reproduction,
 P2 quadrature exactness, P3 grid identities + mpmath cross-check, P4 constant-history
 closed form, P5 pure 2-spin closed form, P6 C(t,t)=1 / R(t,t-)=1, P7 paramagnet + FDT,
 P8 uniform-grid brute force, P9 RK order conditions, P10 the numbers printed in Fig. 7
-(tests/test_oracle_golden.py), P11-P14 Dormand-Prince start-up (tests/test_oracle_dp.py).  "parity unpinned": controller
-tie-breaks (paper silent; readings G20, G25 in DESIGN.md).
+(tests/test_oracle_golden.py), P11-P14 Dormand-Prince start-up (tests/test_oracle_dp.py), P15 the beta0 forcing
+path (equilibrium start beta0 = 1/T is stationary from the first step: mu, E, time-translation invariance, FDT),
+orc_mu_at (cubic reproduction, window placement), the controller constants of PAPER.md:320 on a stubbed error
+sequence.  "parity unpinned": controller tie-breaks and the sparsification schedule (paper silent; readings G20,
+G25 in DESIGN.md).
 """
 from __future__ import annotations
 

@@ -112,6 +112,48 @@ def test_P4_constant_history_closed_form(T, tM):
     d = out["deriv"]
     assert np.abs(d[:, 0] - (-T - tM * om)).max() < 1e-12 * (1 + tM)
     assert np.abs(d[:, 1] - (-(T + 2 * tM) + tM * om)).max() < 1e-12 * (1 + tM)
+    # second-argument equations (readings G9-G11): mu(theta_i t) = T + 2 theta_i t is linear in t, so
+    # the 4-point Lagrange of orc_mu_at reproduces it; d2C = T + t w_i, d2R = T + 2 theta_i t - t w_i,
+    # and the ray derivatives F = d1 + theta_i d2 (Eq.(22))
+    th = grid.theta
+    assert np.abs(d[:, 2] - (T + tM * om)).max() < 1e-12 * (1 + tM)
+    assert np.abs(d[:, 3] - (T + 2 * th * tM - tM * om)).max() < 1e-12 * (1 + tM)
+    assert np.abs(d[:, 4] - (d[:, 0] + th * d[:, 2])).max() < 1e-13 * (1 + tM)
+    assert np.abs(d[:, 5] - (d[:, 1] + th * d[:, 3])).max() < 1e-13 * (1 + tM)
+    assert abs(d[-1, 4]) < 1e-12 * (1 + tM) and abs(d[-1, 5]) < 1e-12 * (1 + tM)   # C(t,t), R(t,t-) stay 1
+
+
+@pytest.mark.parametrize("M", [1, 2, 3, 4, 9, 33])
+def test_mu_at_reproduces_cubics_and_uses_the_new_mu(M):
+    """orc_mu_at (reading G11): local 4-point Lagrange in t over rows k..k+3 with
+    k = clamp(n(tau) - 1, 0, M - 3) and mu_M = the value just computed.  Any cubic in t is
+    reproduced to rounding for every tau in [0, t_M] (fewer rows: degree M); the interpolant goes
+    through the nodes; a lower-order or mis-centred window does not pass."""
+    rng = np.random.default_rng(M)
+    t = np.concatenate([[0.0], np.cumsum(rng.uniform(0.05, 1.5, M))])
+    deg = min(3, M)
+    coef = rng.uniform(-1.0, 1.0, deg + 1)
+    mu_all = np.polyval(coef, t)
+    lib = O._load()
+    taus = np.concatenate([rng.uniform(0.0, t[M], 40), t, [0.5 * (t[M - 1] + t[M])]])
+    for tau in taus:
+        got = lib.orc_mu_at(O._p(t), O._p(mu_all), M, float(tau))
+        assert got == pytest.approx(np.polyval(coef, tau), abs=2e-12 * (1 + t[M]) ** 3)
+    if M >= 4:
+        # not exact one degree above (the window is 4 points) ...
+        quartic = t ** 4
+        tau = 0.5 * (t[M - 1] + t[M])
+        assert abs(lib.orc_mu_at(O._p(t), O._p(quartic), M, float(tau)) - tau ** 4) > 1e-6
+        # ... and the window is rows n-1 .. n+2 around the interval of tau (clamped at both ends):
+        # a spike on a row outside that window leaves the value untouched
+        n = 2 if M >= 6 else 1
+        tau = 0.5 * (t[n] + t[n + 1])
+        base = lib.orc_mu_at(O._p(t), O._p(mu_all), M, float(tau))
+        for far in range(M + 1):
+            spiked = mu_all.copy(); spiked[far] += 1.0
+            moved = lib.orc_mu_at(O._p(t), O._p(spiked), M, float(tau)) != base
+            k = min(max(n - 1, 0), M - 3)
+            assert moved == (k <= far <= k + 3)
 
 
 def test_row_search_brute_force():

@@ -265,3 +265,99 @@ def test_adaptive_run_with_sparsification_is_sane():
     assert N < accepted + 1                          # sparsification removed rows
     assert -0.8867 < H.E[N - 1] < -0.80
     assert all(r[2] <= 2e-6 for r in log if r[3])
+
+
+# ------------------------------------------------------------------------------------ P15
+def _equilibrium_start_run(T=1.0, L=96, s=6, h=0.025, steps=120):
+    grid = O.Grid(L=L, s=s, t_max=20.0)
+    model = O.Model(lam=[0.0, 0.0, 0.0, 1.0], T=T, beta0=1.0 / T)
+    return grid, model, O.run_fixed(grid, model, h, steps)
+
+
+def test_P15_equilibrium_start_is_stationary_from_the_first_step():
+    """The beta0 forcing path (Eq.(12)-(14)): F_C = beta0 f'(C(t,0)) C(t',0) in
+    the C equation, beta0 f'(C(t,0)) C(t,0) in mu, -beta0 f(C(t,0)) in E, and row 0 with
+    mu0 = T + beta0 f'(1) (reading G13).  For beta0 = 1/T in the paramagnet (p = 3, T = 1 > T_d) the
+    system STARTS in equilibrium, so what P7 only reaches as t -> infinity must hold from t = 0:
+      mu(t) = T + f'(1)/T = 2.5,  E(t) = -f(1)/T = -0.5  for every stored row,
+      C(t,t') = C(t-t'), R(t,t') = R(t-t')  (time-translation invariance),
+      T R(tau) = -dC/dtau                     (FDT), from the first rows on.
+    A swapped fc/fc2, a missing beta0 f(C(t,0)) in E, a missing beta0 term in mu or a wrong mu0
+    each move these by O(0.1) (checked by mutating dmfe_oracle.c / History.__init__)."""
+    from scipy.interpolate import CubicSpline
+    T = 1.0
+    grid, model, H = _equilibrium_start_run(T=T)
+    n = H.n_rows
+    assert np.abs(H.mu[:n] - (T + 1.5 / T)).max() < 5e-6
+    assert np.abs(H.E[:n] + 0.5 / T).max() < 2e-6
+    # read C(t, t - tau), R(t, t - tau) off the stored rows with a cubic spline in theta
+    for tau in (0.25, 1.0):
+        vals = []
+        for k in range(1, n):
+            t = H.t[k]
+            if t < tau + 0.25:
+                continue
+            th = 1.0 - tau / t
+            sC, sR = CubicSpline(grid.theta, H.hist[k, :, 0]), CubicSpline(grid.theta, H.hist[k, :, 2])
+            # dC/dtau at fixed t = -(1/t) dC/dtheta
+            vals.append((float(sC(th)), float(sR(th)), float(-sC(th, 1) / t)))
+        vals = np.array(vals)
+        assert len(vals) > 40
+        assert np.ptp(vals[:, 0]) < 2e-5, "C(t, t - tau) depends on t: not stationary"
+        assert np.ptp(vals[:, 1]) < 6e-5, "R(t, t - tau) depends on t: not stationary"
+        assert np.abs(T * vals[:, 1] + vals[:, 2]).max() < 2e-4, "FDT violated"
+        assert 0.2 < vals[0, 0] < 0.95          # not vacuous: the correlation has decayed
+
+
+def test_P15_beta0_zero_is_not_stationary():
+    """Sharpness of P15: the same run from the random start (beta0 = 0) is far from stationary."""
+    grid = O.Grid(L=64, s=4, t_max=20.0)
+    H = O.run_fixed(grid, O.Model(lam=[0.0, 0.0, 0.0, 1.0], T=1.0, beta0=0.0), 0.05, 20)
+    assert abs(H.mu[1] - 2.5) > 0.5 and abs(H.E[1] + 0.5) > 0.2
+
+
+# ------------------------------------------------------------------------------------ controller constants
+def test_controller_constants_from_a_stubbed_error_sequence(monkeypatch):
+    """PAPER.md:320: "the previous ten time steps are reverted and the time step is halved" when
+    eps_RK > 2 eps; otherwise the step is accepted and the next step is reduced to 0.9 h if
+    eps_RK > eps, enlarged to 1.01 h if eps_RK < eps/2 (reading G20); the Eq.(24) cap
+    13.9/(4 sqrt(f''(1))) applies throughout.  The error estimate is stubbed, so only the
+    controller's constants and its bookkeeping are exercised."""
+    grid = O.Grid(L=16, s=4, t_max=20.0)
+    model = O.Model(lam=[0.0, 0.0, 0.0, 1.0], T=1.0)
+    H = O.History(grid, model, 64)
+    eps_list = iter([0.2, 0.4, 0.6, 1.5, 0.5, 1.0, 2.0, 2.0000001] + [0.1] * 14 + [3.0, np.nan, 0.1])
+    monkeypatch.setattr(O, "rk_step", lambda H_, h_: next(eps_list))
+
+    def fake_complete(H_):
+        H_.n_rows += 1
+    monkeypatch.setattr(O, "complete_row", fake_complete)
+    tol, h = 1.0, 0.1
+    cap = 13.9 / (4.0 * np.sqrt(3.0))            # f''(1) = 3 for f = q^3/2
+    assert O.h_stab(model) == pytest.approx(cap, rel=1e-15)
+    got = []
+    for _ in range(25):
+        ok, h, eps = O.controller_step(H, h, tol)
+        got.append((ok, h, H.n_rows))
+    exp, hh, rows = [], 0.1, 1
+    for e in [0.2, 0.4, 0.6, 1.5, 0.5, 1.0, 2.0]:            # all accepted (eps <= 2 tol)
+        rows += 1
+        hh = hh * 0.9 if e > 1.0 else (hh * 1.01 if e < 0.5 else hh)
+        exp.append((True, hh, rows))
+    rows = max(1, rows - 10); hh /= 2.0                        # 2.0000001 > 2 tol: ten rows, h/2
+    exp.append((False, hh, rows))
+    for _ in range(14):
+        rows += 1; hh *= 1.01
+        exp.append((True, hh, rows))
+    rows -= 10; hh /= 2.0                                      # 15 rows -> 5
+    exp.append((False, hh, rows))
+    rows = max(1, rows - 10); hh /= 2.0                        # NaN: reverted too; never below row 0
+    exp.append((False, hh, rows))
+    rows += 1; hh *= 1.01
+    exp.append((True, hh, rows))
+    assert [g[0] for g in got] == [e[0] for e in exp]
+    assert [g[2] for g in got] == [e[2] for e in exp]
+    np.testing.assert_allclose([g[1] for g in got], [e[1] for e in exp], rtol=1e-15)
+    # the cap of Eq.(24)
+    ok, h2, _ = (lambda: (monkeypatch.setattr(O, "rk_step", lambda H_, h_: 0.0), O.controller_step(H, cap, tol))[1])()
+    assert ok and h2 == cap
