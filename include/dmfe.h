@@ -176,19 +176,6 @@ DMFE_API int dmfe_last_kernel_ms(dmfe_ctx *ctx, float *ms);
  * launches themselves, so this can bracket every launch of a timed region. */
 DMFE_API int dmfe_kernel_time_stats(dmfe_ctx *ctx, int32_t *n_launches, double *total_ms, double *min_ms);
 DMFE_API int dmfe_probe_fp64_tflops(dmfe_ctx *ctx, int32_t n_iter, double *tflops, int32_t *sm_count);
-/* Load-path probe: one CTA of `threads` threads per SM; per iteration every
- * warp issues n_loads independent 256-bit loads from an L1-resident buffer with lane pattern
- * 0 coalesced, 1 lane pairs share a cell, 2 broadcast, 3 stencil-like (cell l/4 + (l&3)), 4 one cell
- * per 128-byte line, 5 coalesced with only every fourth lane active, 6 coalesced with 12 scattered
- * lanes active, 7 coalesced with lanes 0..7 active, 8 one cell per line with 12 scattered lanes,
- * 9 the same gathers from shared memory (2 x 128 bit, lane-private pseudo-random cells), 10 no loads
- * but 16 integer multiply-adds per 'load' (issue-slot probe), and n_dfma (multiple of 8) independent
- * DFMAs.  Returns SM cycles per warp-iteration (clock64 around the loop, averaged over SMs).
- * Synchronises.  pattern outside 0..10, n_dfma not a multiple of 8 or threads not a multiple of 32
- * in [32, 1024]: DMFE_EINVAL. */
-DMFE_API int dmfe_probe_load_path(dmfe_ctx *ctx, int32_t pattern, int32_t n_loads, int32_t n_dfma, int32_t threads,
-                         double *cycles_per_warp_iter);
-
 #ifdef __cplusplus
 }
 #endif

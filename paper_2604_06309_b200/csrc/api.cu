@@ -33,6 +33,10 @@ static void free_all(dmfe_ctx *c) {
   cudaFree(c->tab);
   cudaFree(c->blo);
   cudaFree(c->rowtab);
+  cudaFree(c->br);
+  cudaFree(c->jtop);
+  cudaFree(c->coefM);
+  cudaFree(c->coefT);
   cudaFree(c->cur);
   cudaFree(c->scal);
   cudaFree(c->iscal);
@@ -92,6 +96,10 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&c->cur, sizeof(double2) * (size_t)L);
     if (e == cudaSuccess) e = cudaMalloc(&c->blo, sizeof(int32_t) * (size_t)L);
+    if (e == cudaSuccess) e = cudaMalloc(&c->br, sizeof(int2) * (size_t)L);
+    if (e == cudaSuccess) e = cudaMalloc(&c->jtop, sizeof(int32_t) * (size_t)L);
+    if (e == cudaSuccess) e = cudaMalloc(&c->coefM, sizeof(double) * 8 * (size_t)L);
+    if (e == cudaSuccess) e = cudaMalloc(&c->coefT, sizeof(double) * 16 * (size_t)L);
     if (e == cudaSuccess) e = cudaMalloc(&c->scal, sizeof(double) * SC_COUNT);
     if (e == cudaSuccess) e = cudaMalloc(&c->iscal, sizeof(int32_t) * IS_COUNT);
     if (e == cudaSuccess) e = cudaMalloc(&c->rk, sizeof(double) * 8 * (size_t)L);

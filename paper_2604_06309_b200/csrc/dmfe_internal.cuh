@@ -59,6 +59,11 @@ struct dmfe_ctx {
   double2 *cur;     // [L] {C, R} of the current row, packed for 16-byte gathers
   int32_t *blo;     // [L] per-call row bracket table: blo[c] = n(theta_c t_M)
   double2 *rowtab;  // [rowtab_cap] per-call {t_n, 1 / (t_{n+1} - t_n)}
+  // S = 4 only (pairs_s4.cuh), rebuilt per call by the pre-pass
+  int2 *br;         // [L] row bracket of the grid cell of phi2, indexed by the phi2 stencil start
+  int32_t *jtop;    // [L] first node of every target whose type-2 interval is the top one
+  double *coefM;    // [L][8]  centred cubics of {C, R} of the current row, per stencil start
+  double *coefT;    // [L][16] centred cubics of {C, dC, R, dR} of row M-1
   int32_t rowtab_cap;
   double *scal;     // [SC_COUNT]
   int32_t *iscal;   // [IS_COUNT]

@@ -1,0 +1,52 @@
+// Instantiations and launcher of the 4-point-stencil pair kernel (pairs_s4.cuh).
+#include "pairs_s4.cuh"
+
+using namespace dmfe_rhs;
+
+int dmfe_launch_pairs_s4(dmfe_ctx *ctx, const RhsArgs &a, int grid) {
+  const int L = a.L, M = a.M;
+  const long long pairs_cta = (long long)L * L / grid;
+  // shared-memory copies of the packed current row [L] double2 and the row brackets [L-3] int2 and,
+  // when that fits and a CTA has enough pairs to amortise copying M entries, of the row table [M]
+  const size_t smem1 = 24 * (size_t)L, smem2 = smem1 + 16 * (size_t)M;
+  const int mode = (smem2 <= (size_t)ctx->smem_max && 2LL * M <= pairs_cta) ? 2
+                   : (smem1 <= (size_t)ctx->smem_max ? 1 : 0);
+  const size_t smem = mode == 2 ? smem2 : (mode == 1 ? smem1 : 0);
+  const bool hooks = a.out.rows2 != nullptr;
+  // the polynomial degree of f is a compile-time constant for p_max <= 4 (the paper's models
+  // p = 2, 3, 2+4, 3+4, 2+3+4); larger p_max (3+9) takes the run-time Horner loop
+  const int pd = ctx->model.pmax <= 3 ? 3 : (ctx->model.pmax == 4 ? 4 : 0);
+#define DMFE_LAUNCH_K(KFN)                                                                              \
+  do {                                                                                                  \
+    auto kfn = KFN;                                                                                     \
+    if (smem + 4096 > 48 * 1024)                                                                        \
+      CUDA_TRY(ctx, cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+    CUDA_TRY(ctx, launch_pdl(kfn, grid, S4_THREADS, smem, ctx->stream, a, ctx->model));                 \
+  } while (0)
+#define DMFE_LAUNCH_S4(PD_, SM_)                                       \
+  do {                                                                 \
+    if (hooks)                                                         \
+      DMFE_LAUNCH_K((history_integrals_s4_kernel<PD_, SM_, true>));    \
+    else                                                               \
+      DMFE_LAUNCH_K((history_integrals_s4_kernel<PD_, SM_, false>));   \
+  } while (0)
+#define DMFE_LAUNCH_S4M(PD_)   \
+  do {                         \
+    if (mode == 2)             \
+      DMFE_LAUNCH_S4(PD_, 2);  \
+    else if (mode == 1)        \
+      DMFE_LAUNCH_S4(PD_, 1);  \
+    else                       \
+      DMFE_LAUNCH_S4(PD_, 0);  \
+  } while (0)
+  if (pd == 3)
+    DMFE_LAUNCH_S4M(3);
+  else if (pd == 4)
+    DMFE_LAUNCH_S4M(4);
+  else
+    DMFE_LAUNCH_S4M(0);
+#undef DMFE_LAUNCH_S4M
+#undef DMFE_LAUNCH_S4
+#undef DMFE_LAUNCH_K
+  return DMFE_OK;
+}

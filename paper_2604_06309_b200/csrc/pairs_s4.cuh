@@ -1,0 +1,361 @@
+// Pair kernel for the 4-point stencil (S = 4: every configuration of BASELINE.json): the L^2 pairs
+// of one right-hand side (section 3.3-3.4; steps a2-a6, a8 of DESIGN.md).
+//
+// Same mapping as pairs_generic.cuh (persistent CTA per SM, groups of G warps per target, lanes
+// <-> adjacent nodes j) and the same results up to rounding, restructured around what the ncu
+// captures of round 2 showed to bound it (latency of dependent global loads at 16 warps per SM):
+//
+//  1. The top interval is a loop of its own.  tau2 = fl(phi2 t_M) is monotone in j, so for every
+//     target the pairs whose row is n2 = M-1 (upper row = the current row M, quadratic in t,
+//     reading G12) are a suffix j >= jtop[i] of the nodes -- half of all pairs on the log-spaced
+//     workloads, because the quadrature nodes are dense near theta = 1.  That loop needs no row
+//     search, and rows M-1 and M are read through their coefficient forms: the pre-pass turns the
+//     4-point index-Lagrange interpolant of every stencil start a into the cubic in v = u - 3/2
+//     (coefT[a]: {C, dC, R, dR} of row M-1, coefM[a]: {C, R} of row M).  A thread keeps the six
+//     cubics of its last stencil start in registers: psi = theta_i / phi2 moves by less than a grid
+//     cell over the top interval for most targets, so most top pairs load nothing but their table
+//     entries.
+//  2. The general loop (j < jtop[i], n2 <= M-2: both rows complete) finds n2 by probing upward from
+//     the lower end of the bracket br[a2] (n2 - lo is 0 for 85 % of the pairs, <= 2 for 99.9 %),
+//     one pair ahead, while the lower-row cells of the current pair are in flight.
+//  3. Pair-table entries are requested two pairs ahead, type-1 cells one pair ahead.
+#pragma once
+#include <type_traits>
+
+#include "rhs_common.cuh"
+
+namespace dmfe_rhs {
+
+
+// centred fractional coordinate v = u - 3/2 of a packed pair-table entry (dmfe_internal.cuh:
+// u = 16 x - 257 with x the double whose mantissa field is the entry's low 48 bits): exact
+__device__ __forceinline__ double tab_v(uint64_t e) {
+  const uint64_t bits = 0x4030000000000000ULL | (e & 0xFFFFFFFFFFFFULL);
+  return fma(__longlong_as_double((long long)bits), 16.0, -258.5);
+}
+__device__ __forceinline__ int tab_start(uint64_t e) { return (int)(e >> 48); }
+
+__device__ __forceinline__ double cubic(const double4 c, double v) { return fma(fma(fma(c.w, v, c.z), v, c.y), v, c.x); }
+
+// Lagrange cardinal weights on the nodes -3/2, -1/2, 1/2, 3/2 at v (10 FP64 instructions): with
+// a = v^2 - 1/4 and b = v^2 - 9/4:  w0 = a (3/2 - v)/6, w3 = a (3/2 + v)/6, w1 = b (v - 1/2)/2,
+// w2 = -b (v + 1/2)/2 = -(w1 + b/2), w0 = a/2 - w3
+__device__ __forceinline__ void lagrange4_centred(double v, double (&w)[4]) {
+  const double a = fma(v, v, -0.25);
+  const double b = a - 2.0;
+  const double a6 = a * (1.0 / 6.0);
+  const double hb = 0.5 * b;
+  w[3] = a6 * (v + 1.5);
+  w[0] = fma(3.0, a6, -w[3]);
+  w[1] = hb * (v - 0.5);
+  w[2] = -(w[1] + hb);
+}
+
+// A factor (Eq.(18)): {C, R} of the current row at the coordinate of a pair-table
+// entry, 4-point index-Lagrange on the packed row (shared memory when SM >= 1)
+__device__ __forceinline__ double2 a_factor(const double2 *cur, uint64_t e) {
+  const int a = tab_start(e);
+  const double v = tab_v(e);
+  double w[4];
+  lagrange4_centred(v, w);
+  const double2 y0 = cur[a], y1 = cur[a + 1], y2 = cur[a + 2], y3 = cur[a + 3];
+  return make_double2(fma(w[3], y3.x, fma(w[2], y2.x, fma(w[1], y1.x, w[0] * y0.x))),
+                      fma(w[3], y3.y, fma(w[2], y2.y, fma(w[1], y1.y, w[0] * y0.y))));
+}
+
+template <int PD, int SM, bool HOOKS>
+__global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(RhsArgs a, ModelCoef mc) {
+  // SM: 0 = per-call tables read from global memory, 1 = cur and br in shared memory, 2 = rowtab too
+  constexpr bool SMT = SM >= 1, SMR = SM == 2;
+  extern __shared__ double4 smem_dyn[];
+  pdl_launch_dependents();
+  pdl_wait();
+  const int L = a.L, M = a.M;
+  const double2 *cur = a.cur;
+  const double2 *rowtab = a.rowtab;
+  const int2 *br = a.br;
+  if (SMT) {
+    double2 *s_cur = reinterpret_cast<double2 *>(smem_dyn);
+    double2 *s_row = s_cur + L;
+    int2 *s_br = reinterpret_cast<int2 *>(s_row + (SMR ? M : 0));
+    for (int k = threadIdx.x; k < L; k += S4_THREADS) s_cur[k] = a.cur[k];
+    for (int k = threadIdx.x; k < L - 3; k += S4_THREADS) s_br[k] = a.br[k];
+    if (SMR)
+      for (int k = threadIdx.x; k < M; k += S4_THREADS) s_row[k] = a.rowtab[k];
+    __syncthreads();
+    cur = s_cur, br = s_br;
+    if (SMR) rowtab = s_row;
+  }
+  __shared__ double red[2][S4_THREADS / 32][8];
+
+  const int G = a.G;
+  const int TG = 32 * G;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int group = warp / G, wg = warp % G;
+  const int ngroups = (S4_THREADS / 32) / G;
+  const int tig = wg * 32 + lane;
+  const size_t plane = (size_t)L * (size_t)L;
+  const double tM = a.t[M];
+  // top interval [t_{M-1}, t_M]: the same for every pair that falls into it
+  const double2 rtT = a.rowtab[M - 1];
+  const double4 *__restrict__ coefM = a.coefM;
+  const double4 *__restrict__ coefT = a.coefT;
+  const double4 *__restrict__ hist = a.hist;
+  const int K = (tig < L) ? (L - tig + TG - 1) / TG : 0;  // pairs j = tig + k TG of this thread
+  int parity = 0;
+
+  for (int i = blockIdx.x * ngroups + group; i < L; i += gridDim.x * ngroups, parity ^= 1) {
+    const double th_i = a.theta[i], om_i = a.omega[i];
+    const double tau1 = __dmul_rn(th_i, tM);
+    const int n1 = a.blo[i];
+    const bool top1 = (n1 + 1 == M);
+    double h1[4];
+    {
+      const double2 rt = rowtab[n1];
+      t_weights(rt.x, rt.y, tau1, top1, h1);
+    }
+
+    // ================= type-1 half of Eq.(21): S1, S3, S5, S6 =================
+    // Pipeline: the pair-table entry two pairs ahead, nu_j and the two cells one pair ahead.  When
+    // row n1 + 1 is the current row M (top interval of the type-1 lookup) its values come from the
+    // packed current row and carry no slope (reading G12): the history's row M is never read here.
+    auto type1 = [&](auto top1_c) {
+      constexpr bool TOP1 = decltype(top1_c)::value;
+      double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+      const uint64_t *pt = a.tab + (size_t)i * (size_t)L + tig;  // entry of pair k
+      const double4 *pc = hist + (size_t)n1 * (size_t)L + tig;   // lower cell of pair k
+      const double *pn = a.nu + tig;
+      const double2 *pu = cur + tig;
+      uint64_t e_c = 0, e_n = 0;
+      double nu_c = 0.0;
+      double4 lo_c = make_double4(0, 0, 0, 0), hi_c = lo_c;
+      if (K > 0) {
+        e_c = ld_stream(pt);
+        nu_c = *pn;
+        lo_c = ld_cell(pc);
+        if (TOP1) {
+          const double2 c = *pu;
+          hi_c = make_double4(c.x, 0.0, c.y, 0.0);
+        } else {
+          hi_c = ld_cell(pc + L);
+        }
+      }
+      if (K > 1) e_n = ld_stream(pt + TG);
+#pragma unroll 2
+      for (int k = 0; k < K; ++k) {
+        uint64_t e_nn = 0;
+        double nu_n = 0.0;
+        double4 lo_n = make_double4(0, 0, 0, 0), hi_n = lo_n;
+        pt += TG, pc += TG, pn += TG, pu += TG;
+        if (k + 2 < K) e_nn = ld_stream(pt + TG);
+        if (k + 1 < K) {
+          nu_n = *pn;
+          lo_n = ld_cell(pc);
+          if (TOP1) {
+            const double2 c = *pu;
+            hi_n = make_double4(c.x, 0.0, c.y, 0.0);
+          } else {
+            hi_n = ld_cell(pc + L);
+          }
+        }
+        const double2 A1 = a_factor(cur, e_c);
+        const double C1 = A1.x, R1 = A1.y;
+        const double B1C = TOP1 ? h1[0] * lo_c.x + h1[1] * lo_c.y + h1[2] * hi_c.x
+                                : h1[0] * lo_c.x + h1[1] * lo_c.y + h1[2] * hi_c.x + h1[3] * hi_c.y;
+        const double B1R = TOP1 ? h1[0] * lo_c.z + h1[1] * lo_c.w + h1[2] * hi_c.z
+                                : h1[0] * lo_c.z + h1[1] * lo_c.w + h1[2] * hi_c.z + h1[3] * hi_c.w;
+        const double nR1 = nu_c * R1, nB1R = nu_c * B1R;
+        acc0 = fma(f2<PD>(mc, C1) * nR1, B1C, acc0);   // S1: K(t,s) C(t',s)
+        acc1 = fma(f1<PD>(mc, C1), nB1R, acc1);        // S3: D(t,s) R(t',s)
+        acc2 = fma(f2<PD>(mc, B1C) * nB1R, C1, acc2);  // S5: K(t',s) C(t,s)
+        acc3 = fma(f1<PD>(mc, B1C), nR1, acc3);        // S6: D(t',s) R(t,s)
+        e_c = e_n, e_n = e_nn, nu_c = nu_n, lo_c = lo_n, hi_c = hi_n;
+      }
+      const double acc[4] = {acc0, acc1, acc2, acc3};
+      constexpr int slot[4] = {0, 2, 4, 5};
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        double v = acc[q];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[parity][warp][slot[q]] = v;
+      }
+    };
+    if (top1)
+      type1(std::true_type{});
+    else
+      type1(std::false_type{});
+
+    // ================= type-2 half: S2, S4, S7, S8 =================
+    {
+      double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+      const int jt = a.jtop[i];
+      int Kg = (jt > tig) ? (jt - tig + TG - 1) / TG : 0;  // this thread's pairs with j < jtop[i]
+      if (Kg > K) Kg = K;
+      const uint64_t *pt2 = a.tab + plane + (size_t)i * (size_t)L + tig;  // phi2 entry of pair k
+      const uint64_t *pt3 = pt2 + plane;                                   // psi entry of pair k
+      const double2 *pn = a.thnu + tig;                                    // {theta_j, nu_j}
+      auto finish = [&](double nj, double C2, double R2, double B2C, double B2R) {
+        const double nR2 = nj * R2;
+        const double K2 = f2<PD>(mc, C2) * nR2;
+        acc0 = fma(K2, B2C, acc0);                     // S2: K(t,s) C(s,t')
+        acc1 = fma(K2, B2R, acc1);                     // S4: K(t,s) R(s,t')
+        acc2 = fma(f1<PD>(mc, B2C), nR2, acc2);        // S7: D(s,t') R(t,s)
+        acc3 = fma(nR2, f2<PD>(mc, B2C) * B2R, acc3);  // S8: R(t,s) K(s,t')
+      };
+      // entries of pairs k (c) and k + 1 (n); the loops request those of pair k + 2
+      uint64_t e2_c = 0, e3_c = 0, e2_n = 0, e3_n = 0;
+      double2 tn_c = make_double2(0.0, 0.0), tn_n = tn_c;
+      if (K > 0) {
+        e2_c = ld_stream(pt2);
+        e3_c = ld_stream(pt3);
+        tn_c = *pn;
+      }
+      if (K > 1) {
+        e2_n = ld_stream(pt2 + TG);
+        e3_n = ld_stream(pt3 + TG);
+        tn_n = pn[TG];
+      }
+      int k = 0;
+      // ---- general pairs (j < jtop[i]: n2 <= M-2, both rows complete): row search, theta-stencil
+      // on the cells of rows n2 and n2 + 1, cubic Hermite in t.  Index stage (the integer half of
+      // Eq.(20)) one pair ahead: tau2 = fl(phi2 t_M); n2 = max{n : t_n <= tau2} lies
+      // in the bracket br[a2] = [lo, hi] of the grid cell of phi2 and is found by probing upward
+      // from lo (same predicate as a bisection).
+      if (Kg > 0) {
+        int n2_c;
+        double tau2_c;
+        double2 rt_c;
+        {
+          tau2_c = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn_c.x)), tM);
+          const int2 b = br[tab_start(e2_c)];
+          int n = b.x;
+          while (n < b.y && rowtab[n + 1].x <= tau2_c) ++n;
+          n2_c = n;
+          rt_c = rowtab[n];
+        }
+#pragma unroll 2
+        for (; k < Kg; ++k) {
+          const int a3 = tab_start(e3_c);
+          const double4 *p2 = hist + ((size_t)n2_c * (size_t)L + (size_t)a3);
+          double4 x[4];
+#pragma unroll
+          for (int l = 0; l < 4; ++l) x[l] = ld_cell(p2 + l);
+          // index stage of pair k + 1 while the cells arrive
+          int n2_n = 0;
+          double tau2_n = 0.0;
+          double2 rt_n = make_double2(0.0, 0.0);
+          if (k + 1 < Kg) {
+            tau2_n = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn_n.x)), tM);
+            const int2 b = br[tab_start(e2_n)];
+            int n = b.x;
+            while (n < b.y && rowtab[n + 1].x <= tau2_n) ++n;
+            n2_n = n;
+            rt_n = rowtab[n];
+          }
+          uint64_t e2_nn = 0, e3_nn = 0;
+          double2 tn_nn = make_double2(0.0, 0.0);
+          pt2 += TG, pt3 += TG, pn += TG;
+          if (k + 2 < K) {
+            e2_nn = ld_stream(pt2 + TG);
+            e3_nn = ld_stream(pt3 + TG);
+            tn_nn = pn[TG];
+          }
+          if (HOOKS && a.out.rows2) a.out.rows2[(size_t)i * (size_t)L + (size_t)(tig + k * TG)] = n2_c;
+          const double v3 = tab_v(e3_c);
+          double h2[4];
+          t_weights(rt_c.x, rt_c.y, tau2_c, false, h2);
+          double w[4];
+          lagrange4_centred(v3, w);
+          double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
+#pragma unroll
+          for (int l = 0; l < 4; ++l) {
+            cl = fma(w[l], x[l].x, cl);
+            dcl = fma(w[l], x[l].y, dcl);
+            rl = fma(w[l], x[l].z, rl);
+            drl = fma(w[l], x[l].w, drl);
+          }
+#pragma unroll
+          for (int l = 0; l < 4; ++l) {
+            const double4 y = ld_cell(p2 + L + l);
+            cu = fma(w[l], y.x, cu);
+            dcu = fma(w[l], y.y, dcu);
+            ru = fma(w[l], y.z, ru);
+            dru = fma(w[l], y.w, dru);
+          }
+          const double2 A2 = a_factor(cur, e2_c);
+          const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
+          const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
+          finish(tn_c.y, A2.x, A2.y, B2C, B2R);
+          e2_c = e2_n, e3_c = e3_n, tn_c = tn_n;
+          e2_n = e2_nn, e3_n = e3_nn, tn_n = tn_nn;
+          n2_c = n2_n, tau2_c = tau2_n, rt_c = rt_n;
+        }
+      }
+      // ---- top pairs (j >= jtop[i]: n2 = M-1): rows M-1 and M through their coefficient forms,
+      // quadratic in t (reading G12): B = (1 - u^2) Y_{M-1} + d (1 - u) Y'_{M-1} + u^2 Y_M.  The six
+      // cubics of the last stencil start stay in registers (psi moves slowly over the top interval).
+      {
+        int a3_held = -1;
+        double4 qc = make_double4(0, 0, 0, 0), qdc = qc, qr = qc, qdr = qc, uc = qc, ur = qc;
+#pragma unroll 2
+        for (; k < K; ++k) {
+          const int a3 = tab_start(e3_c);
+          if (a3 != a3_held) {
+            qc = ld_cell(coefT + 4 * a3), qdc = ld_cell(coefT + 4 * a3 + 1);
+            qr = ld_cell(coefT + 4 * a3 + 2), qdr = ld_cell(coefT + 4 * a3 + 3);
+            uc = ld_cell(coefM + 2 * a3), ur = ld_cell(coefM + 2 * a3 + 1);
+            a3_held = a3;
+          }
+          const double v3 = tab_v(e3_c);
+          const double2 A2 = a_factor(cur, e2_c);
+          const double2 tn = tn_c;
+          uint64_t e2_nn = 0, e3_nn = 0;
+          double2 tn_nn = make_double2(0.0, 0.0);
+          pt2 += TG, pt3 += TG, pn += TG;
+          if (k + 2 < K) {
+            e2_nn = ld_stream(pt2 + TG);
+            e3_nn = ld_stream(pt3 + TG);
+            tn_nn = pn[TG];
+          }
+          if (HOOKS && a.out.rows2) a.out.rows2[(size_t)i * (size_t)L + (size_t)(tig + k * TG)] = M - 1;
+          const double tau2 = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn.x)), tM);
+          const double d = tau2 - rtT.x;
+          const double u = d * rtT.y;
+          const double q2 = u * u;
+          const double q0 = 1.0 - q2;
+          const double q1 = d * (1.0 - u);
+          const double B2C = fma(q0, cubic(qc, v3), fma(q1, cubic(qdc, v3), q2 * cubic(uc, v3)));
+          const double B2R = fma(q0, cubic(qr, v3), fma(q1, cubic(qdr, v3), q2 * cubic(ur, v3)));
+          finish(tn.y, A2.x, A2.y, B2C, B2R);
+          e2_c = e2_n, e3_c = e3_n, tn_c = tn_n;
+          e2_n = e2_nn, e3_n = e3_nn, tn_n = tn_nn;
+        }
+      }
+      const double acc[4] = {acc0, acc1, acc2, acc3};
+      constexpr int slot[4] = {1, 3, 6, 7};
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        double v = acc[q];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[parity][warp][slot[q]] = v;
+      }
+    }
+    if (G > 1)
+      group_barrier(1 + group, TG);
+    else
+      __syncwarp();
+    if (tig == 0) {
+      // C(theta_i t, 0) = the type-1 lookup at node j = 0, needed by the beta0 forcing (Eq.(12))
+      double b1c_first = 0.0;
+      if (mc.beta0 != 0.0) {
+        const double4 lo = hist[(size_t)n1 * (size_t)L];
+        double4 hi = make_double4(cur[0].x, 0.0, cur[0].y, 0.0);
+        if (!top1) hi = hist[(size_t)(n1 + 1) * (size_t)L];
+        b1c_first = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
+      }
+      combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur);
+    }
+  }
+}
+
+}  // namespace dmfe_rhs

@@ -13,8 +13,7 @@ from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_int, c_int32
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# DMFE_LIBRARY: load another build of the same library (kernel tuning experiments)
-LIB_PATH = os.environ.get("DMFE_LIBRARY") or os.path.join(_HERE, "libdmfe.so")
+LIB_PATH = os.path.join(_HERE, "libdmfe.so")
 
 DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE, DMFE_ENOMEM = 0, -1, -2, -3, -4, -5, -6
 
@@ -22,7 +21,7 @@ EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror
            "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_init_state", "dmfe_rk_step",
            "dmfe_dp_step", "dmfe_set_step_size",
            "dmfe_sparsify", "dmfe_set_sparsify_threshold", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
-           "dmfe_probe_fp64_tflops", "dmfe_probe_load_path"]
+           "dmfe_probe_fp64_tflops"]
 
 
 class dmfe_params(Structure):
@@ -89,8 +88,6 @@ def load_library():
     lib.dmfe_sparsify.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32), c_void_p]
     lib.dmfe_set_sparsify_threshold.restype = c_int
     lib.dmfe_set_sparsify_threshold.argtypes = [c_void_p, c_double]
-    lib.dmfe_probe_load_path.restype = c_int
-    lib.dmfe_probe_load_path.argtypes = [c_void_p, c_int32, c_int32, c_int32, c_int32, POINTER(c_double)]
     lib.dmfe_enable_timing.restype = c_int
     lib.dmfe_enable_timing.argtypes = [c_void_p, c_int32]
     lib.dmfe_last_kernel_ms.restype = c_int
@@ -244,14 +241,6 @@ def dmfe_kernel_time_stats(ctx):
     n, tot, mn = c_int32(0), c_double(0.0), c_double(0.0)
     _check(load_library().dmfe_kernel_time_stats(ctx, byref(n), byref(tot), byref(mn)), "dmfe_kernel_time_stats", ctx)
     return n.value, tot.value, mn.value
-
-
-def dmfe_probe_load_path(ctx, pattern, n_loads, n_dfma, threads=512):
-    """-> SM cycles per warp-iteration of the load-path probe (include/dmfe.h)."""
-    out = c_double(0.0)
-    _check(load_library().dmfe_probe_load_path(ctx, pattern, n_loads, n_dfma, threads, byref(out)),
-           "dmfe_probe_load_path", ctx)
-    return out.value
 
 
 def dmfe_probe_fp64_tflops(ctx, n_iter=1 << 16):
