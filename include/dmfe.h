@@ -38,7 +38,7 @@ extern "C" {
 #define DMFE_OK 0
 #define DMFE_EINVAL (-1)      /* bad parameter (L < 2s, t_max <= e, n_rows < 2, NULL pointer ...) */
 #define DMFE_ECUDA (-2)       /* a CUDA call failed; dmfe_last_cuda_error() has the code          */
-#define DMFE_ECAPACITY (-3)   /* append with n_rows == n_cap, or a forced sparsify freed nothing  */
+#define DMFE_ECAPACITY (-3)   /* a step needs a free row: n_rows + 1 > n_cap                      */
 #define DMFE_ESTEPMIN (-4)    /* controller drove h below h_min                    */
 #define DMFE_ENONFINITE (-5)  /* eps_RK not finite and nothing left to revert                     */
 #define DMFE_ENOMEM (-6)      /* host or device allocation failed                                 */
@@ -114,7 +114,7 @@ DMFE_API int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const do
 /* Device-resident integrator state.  The arrays are caller-owned DEVICE memory. */
 typedef struct {
   int32_t n_rows;  /* complete rows (value + derivative + mu); updated by the library            */
-  int32_t n_cap;   /* capacity; a step needs n_rows + 1 <= n_cap - 1                              */
+  int32_t n_cap;   /* capacity; a step needs n_rows + 1 <= n_cap                                  */
   double *t;       /* [n_cap]                                                                     */
   double *mu;      /* [n_cap]                                                                     */
   double *energy;  /* [n_cap] E(t_n) of every stored row                                          */
@@ -128,14 +128,34 @@ typedef struct {
  * sets n_rows = 1 and h = h0 (capped by the stability bound of Eq.(24)). */
 DMFE_API int dmfe_init_state(dmfe_ctx *ctx, dmfe_state *st, double h0);
 
-/* One SSPRK(10,4) step from the last row, all stages on the device.
- * fixed_step != 0: no controller, the row is always appended.  Otherwise the controller of
- * PAPER.md:320 (G20): eps_RK > 2 tol or non-finite -> drop the last 10 rows, h/2, *accepted = 0;
- * else append, h *= 0.9 if eps_RK > tol, h *= 1.01 if eps_RK < tol/2, *accepted = 1.
- * Exactly one scalar record (128 bytes) returns to the host per call; it is read as soon as the
- * pre-pass of the last stage has taken the decision, so on return the evaluation that completes
- * the appended row (its derivative, mu, E) may still be running on the context's stream: work
- * queued on that stream is ordered behind it, other streams must synchronise with it. */
+/* What comes back from a batch of steps (one device-to-host copy per batch). */
+typedef struct {
+  int32_t steps;         /* steps attempted (fewer than asked if the batch stopped or would outgrow n_cap) */
+  int32_t accepted;      /* of which accepted ...                                                        */
+  int32_t reverted;      /* ... and reverted (each drops the last ten rows)                */
+  int32_t n_rows;        /* complete rows after the batch                                                 */
+  int32_t last_accepted; /* decision of the last step                                                     */
+  double t_last;         /* time of the last complete row                                                 */
+  double h_next;         /* step size the controller proposes for the next step                           */
+  double eps_rk;         /* Eq.(25) of the last attempted step                                            */
+} dmfe_advance_result;
+
+/* n_steps SSPRK(10,4) steps from the last row without returning to the host: the
+ * row count, the step size and every decision live in device memory, and one step (ten stage updates
+ * + evaluations and the commit of the decision) is one CUDA graph that is re-launched n_steps times.
+ * fixed_step != 0: no controller, every row is appended.  Otherwise the controller of PAPER.md:320
+ * (G20) runs on the device after every step: eps_RK > 2 tol or non-finite -> drop the last 10 rows,
+ * h/2; else append, h *= 0.9 if eps_RK > tol, h *= 1.01 if eps_RK < tol/2; always h <= the cap of
+ * Eq.(24).  The batch is cut to n_cap - n_rows steps so that it cannot outgrow the arrays (nothing
+ * to do: DMFE_ECAPACITY).  A step that ends with h < h_min (DMFE_ESTEPMIN) or with a non-finite
+ * error and nothing left to revert (DMFE_ENONFINITE) turns the rest of the batch into no-ops and is
+ * returned as the call's code; st and *res describe the state at that point.
+ * step_log: optional HOST [n_steps][4] doubles {accepted, eps_RK, h_next, n_rows after} per step.
+ * Synchronises on the context's stream. */
+DMFE_API int dmfe_advance(dmfe_ctx *ctx, dmfe_state *st, int32_t n_steps, int32_t fixed_step,
+                          dmfe_advance_result *res, double *step_log);
+
+/* One step: dmfe_advance(ctx, st, 1, fixed_step, ...) with *accepted = the decision. */
 DMFE_API int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *accepted);
 
 /* One Dormand-Prince 5(4) step (the start-up integrator "at short times", textbook

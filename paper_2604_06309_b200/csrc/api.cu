@@ -32,6 +32,7 @@ static void free_all(dmfe_ctx *c) {
   cudaFree(c->thnu);
   cudaFree(c->tab);
   cudaFree(c->blo);
+  cudaFree(c->muw);
   cudaFree(c->rowtab);
   cudaFree(c->br);
   cudaFree(c->jtop);
@@ -53,8 +54,10 @@ static void free_all(dmfe_ctx *c) {
   for (int k = 0; k < 2 * c->ev_made; ++k) cudaEventDestroy(c->ev[k]);
   if (c->h_scal) cudaFreeHost(c->h_scal);
   if (c->h_iscal) cudaFreeHost(c->h_iscal);
-  if (c->side) cudaStreamDestroy(c->side);
-  if (c->ev_decided) cudaEventDestroy(c->ev_decided);
+  if (c->step_exec) cudaGraphExecDestroy(c->step_exec);
+  if (c->step_graph) cudaGraphDestroy(c->step_graph);
+  cudaFree(c->steplog);
+  if (c->h_steplog) cudaFreeHost(c->h_steplog);
 }
 
 int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_ctx **out) {
@@ -96,6 +99,7 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
     cudaError_t e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(&c->cur, sizeof(double2) * (size_t)L);
     if (e == cudaSuccess) e = cudaMalloc(&c->blo, sizeof(int32_t) * (size_t)L);
+    if (e == cudaSuccess) e = cudaMalloc(&c->muw, sizeof(double2) * (size_t)L);
     if (e == cudaSuccess) e = cudaMalloc(&c->br, sizeof(int2) * (size_t)L);
     if (e == cudaSuccess) e = cudaMalloc(&c->jtop, sizeof(int32_t) * (size_t)L);
     if (e == cudaSuccess) e = cudaMalloc(&c->coefM, sizeof(double) * 8 * (size_t)L);
@@ -105,8 +109,6 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
     if (e == cudaSuccess) e = cudaMalloc(&c->rk, sizeof(double) * 8 * (size_t)L);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_scal, sizeof(double) * SC_COUNT);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_iscal, sizeof(int32_t) * IS_COUNT);
-    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_decided, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->scal, 0, sizeof(double) * SC_COUNT, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->iscal, 0, sizeof(int32_t) * IS_COUNT, c->stream);
     if (e != cudaSuccess) {

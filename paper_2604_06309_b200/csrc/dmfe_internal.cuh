@@ -31,6 +31,7 @@ enum {
   SC_T0 = 4,     // t_N at the start of the step
   SC_HNEXT = 5,  // step size proposed by the controller (latched into SC_H by stage 0 of the next step)
   SC_ACCEPT = 6, // accept flag of the last step as a double (so that one copy returns the whole record)
+  SC_TLAST = 7,  // time of the last complete row after the last committed step
   SC_COUNT = 16
 };
 // device int block (ctx->iscal)
@@ -38,6 +39,10 @@ enum {
   IS_ACCEPT = 0,  // 1 accepted, 0 reverted
   IS_NROWS = 1,   // complete rows after the step / after sparsify
   IS_FIRST = 2,   // sparsify: first row that moves
+  IS_STATUS = 3,  // 0, or the DMFE_E* code that stopped a batch of steps (later steps of the batch are no-ops)
+  IS_NACC = 4,    // accepted / reverted / attempted steps of the running dmfe_advance call
+  IS_NREV = 5,
+  IS_STEP = 6,
   IS_COUNT = 8
 };
 
@@ -58,6 +63,7 @@ struct dmfe_ctx {
   // ---- O(L) scratch (device) ----
   double2 *cur;     // [L] {C, R} of the current row, packed for 16-byte gathers
   int32_t *blo;     // [L] per-call row bracket table: blo[c] = n(theta_c t_M)
+  double2 *muw;     // [L] per call: mu(theta_c t_M) = muw.x + muw.y * mu(t_M)  (reading G11)
   double2 *rowtab;  // [rowtab_cap] per-call {t_n, 1 / (t_{n+1} - t_n)}
   // S = 4 only (pairs_s4.cuh), rebuilt per call by the pre-pass
   int2 *br;         // [L] row bracket of the grid cell of phi2, indexed by the phi2 stencil start
@@ -86,10 +92,15 @@ struct dmfe_ctx {
   // pinned host scalars for the one-record-per-step readback
   double *h_scal;
   int32_t *h_iscal;
-  // the record is copied on a side stream as soon as the last stage's pre-pass has taken the
-  // decision, while the evaluation that completes the appended row still runs on `stream`
-  cudaStream_t side;
-  cudaEvent_t ev_decided;
+  // one SSPRK(10,4) step as a CUDA graph (21 kernel nodes), re-launched for every step of
+  // dmfe_advance; all of its arguments live in device memory, so it is captured once per state
+  cudaGraph_t step_graph;
+  cudaGraphExec_t step_exec;
+  const void *graph_key[5];  // t, mu, energy, hist pointers of the state it was captured for + flags
+  int graph_off;             // capture failed once: plain launches from then on
+  double *steplog;           // [steplog_cap][4] device: {accepted, eps_RK, h_next, n_rows} per step
+  double *h_steplog;         // pinned host copy
+  int32_t steplog_cap;
 };
 
 #define CUDA_TRY(ctx, call)                              \
@@ -135,14 +146,17 @@ DMFE_HD void dmfe_tab_decode(uint64_t e, int32_t *start, double *frac) {
 // it (rk_step.cu fills this in; k < 0 = no stage update, plain evaluation of row M).
 struct dmfe_stage {
   int32_t k;           // stage 0..9 of PAPER.md:314-316; the update writes the value slots of row N+1
-  int32_t N;           // last complete row
+  int32_t N;           // last complete row (host value; ignored when dev_rows is set)
   int32_t fixed_step;  // k == 9: 1 = no controller
+  int32_t complete;    // the evaluation completes the appended row M: mu[M], energy[M], derivative slots
   double tol, cap;     // k == 9: epsilon of Eq.(25), step cap of Eq.(24)
   double *hist, *t;    // writable views of the caller's history
+  double *mu, *energy; // complete != 0: writable per-row arrays
   double *rk;          // [4][2L]: q1, q2, delta, F
   double *scal;
   int32_t *iscal;
-  cudaEvent_t after_prepass;  // optional: recorded on the stream between the pre-pass and the pair kernel
+  const int32_t *dev_rows;  // device-resident step: number of complete rows (= M) is read from here and
+                            // a non-zero iscal[IS_STATUS] turns the launch into a no-op
 };
 
 // tables.cu

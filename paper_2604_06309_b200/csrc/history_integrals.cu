@@ -19,6 +19,7 @@ namespace {
 using namespace dmfe_rhs;
 
 constexpr int PREP_THREADS = 1024;
+constexpr int PREP_SCUR = 2048;  // block 0 keeps the packed current row in shared memory up to this L
 
 // ---------------------------------------------------------------------------------------------
 // O(L + M) pre-pass, optionally preceded by one SSPRK(10,4) stage update that
@@ -64,10 +65,16 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
                                                                const double4 *hist, double2 *__restrict__ cur,
                                                                double2 *__restrict__ rowtab,
                                                                int32_t *__restrict__ blo, double *scal,
-                                                               PrepS4 s4) {
+                                                               const double *__restrict__ mu_hist,
+                                                               double2 *__restrict__ muw, PrepS4 s4) {  // M, sg: by value, adjusted below
   __shared__ double sm[32], se[32];
   pdl_launch_dependents();
   pdl_wait();
+  if (sg.dev_rows) {  // device-resident step: the row count lives on the device (rk_step.cu)
+    if (sg.iscal[IS_STATUS] != 0) return;
+    M = sg.dev_rows[0];
+    sg.N = M - 1;
+  }
   const int k = sg.k;
   // time of the row being evaluated.  The step size of stage 0 is the controller's proposal
   // (SC_HNEXT); block 0 latches it into SC_H, which stages 1..9 read.
@@ -90,8 +97,30 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
         rowtab[e] = make_double2(tn, 1.0 / (tn1 - tn));
       } else if (e < M + L) {
         const int c = e - M;
-        const int n = row_search_from(t, M - 1, blo[c], __dmul_rn(theta[c], tM));
+        const double tau1 = __dmul_rn(theta[c], tM);
+        const int n = row_search_from(t, M - 1, blo[c], tau1);
         blo[c] = n;
+        {
+          // mu(theta_c t_M): local 4-point Lagrange in t over rows k0..k0+3 (reading G11); the last point
+          // may be the current row M, whose mu is being reduced by block 0: keep its weight apart
+          const int npts = (M + 1 < 4) ? M + 1 : 4;
+          int k0 = n - 1;
+          if (k0 > M + 1 - npts) k0 = M + 1 - npts;
+          if (k0 < 0) k0 = 0;
+          double tq[4];
+          for (int q = 0; q < npts; ++q) tq[q] = (k0 + q == M) ? tM : t[k0 + q];
+          double part = 0.0, wM = 0.0;
+          for (int p = 0; p < npts; ++p) {
+            double wgt = 1.0;
+            for (int q = 0; q < npts; ++q)
+              if (q != p) wgt *= (tau1 - tq[q]) / (tq[p] - tq[q]);
+            if (k0 + p == M)
+              wM = wgt;
+            else
+              part += wgt * mu_hist[k0 + p];
+          }
+          muw[c] = make_double2(part, wM);
+        }
         if (s4.on) {
           // l* = a + 1 for an unclamped start a (S/2 - 1 = 1): clo(a) = a + 1, chi(a) = a + 2; clamped
           // starts: a = 0 -> l* in {0, 1}: [blo[0], blo[2]]; a = L-4 -> l* in {L-3 .. L-1}: [blo[L-3], blo[L-1]]
@@ -136,6 +165,7 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
   double4 *rowM = const_cast<double4 *>(hist) + (size_t)M * (size_t)L;
   double eacc = 0.0, am = 0.0, ae = 0.0;
   __shared__ double s_c0;
+  __shared__ double2 s_cur[PREP_SCUR];
   for (int l = threadIdx.x; l < L; l += blockDim.x) {
     double2 y;  // {C, R} of row M at node l
     if (k >= 0) {
@@ -178,6 +208,7 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
       y = make_double2(c.x, c.z);
     }
     cur[l] = y;
+    if (l < PREP_SCUR) s_cur[l] = y;
     if (l == 0) s_c0 = y.x;
     const double fp = horner(mc.c1, mc.pmax - 1, y.x), fpp = horner(mc.c2, mc.pmax - 2, y.x);
     const double nj = nu[l];
@@ -190,8 +221,9 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
   }
   if (s4.on) {  // coefficient form of the row just packed (block-wide: a start needs four neighbours)
     __syncthreads();
+    const double2 *src = (L <= PREP_SCUR) ? s_cur : cur;  // small L: no round trip through L2
     for (int a = threadIdx.x; a < L - 3; a += blockDim.x) {
-      const double2 y0 = cur[a], y1 = cur[a + 1], y2 = cur[a + 2], y3 = cur[a + 3];
+      const double2 y0 = src[a], y1 = src[a + 1], y2 = src[a + 2], y3 = src[a + 3];
       s4.coefM[2 * (size_t)a] = centred_cubic(y0.x, y1.x, y2.x, y3.x);
       s4.coefM[2 * (size_t)a + 1] = centred_cubic(y0.y, y1.y, y2.y, y3.y);
     }
@@ -205,9 +237,16 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
   __shared__ double sx[32];
   if ((threadIdx.x & 31) == 0) sm[w] = am, se[w] = ae, sx[w] = eacc;
   __syncthreads();
-  if (threadIdx.x == 0) {
-    double tm = 0.0, te = 0.0, eps = 0.0;
-    for (int q = 0; q < nw; ++q) tm += sm[q], te += se[q], eps += sx[q];
+  if (threadIdx.x < 32) {  // second level: the first warp adds the warp sums (fixed order)
+    double tm = threadIdx.x < nw ? sm[threadIdx.x] : 0.0;
+    double te = threadIdx.x < nw ? se[threadIdx.x] : 0.0;
+    double eps = threadIdx.x < nw ? sx[threadIdx.x] : 0.0;
+    for (int o = 16; o > 0; o >>= 1) {
+      tm += __shfl_xor_sync(0xffffffffu, tm, o);
+      te += __shfl_xor_sync(0xffffffffu, te, o);
+      eps += __shfl_xor_sync(0xffffffffu, eps, o);
+    }
+    if (threadIdx.x == 0) {
     const double c0 = s_c0;
     scal[SC_MU] = mc.T + tM * tm + mc.beta0 * horner(mc.c1, mc.pmax - 1, c0) * c0;
     scal[SC_E] = -tM * te - mc.beta0 * horner(mc.c0, mc.pmax, c0);
@@ -227,10 +266,11 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
           hn = fmin(hn, sg.cap);
         }
       }
-      scal[SC_EPS] = eps;
-      scal[SC_HNEXT] = hn;
-      scal[SC_ACCEPT] = (double)accept;
-      sg.iscal[IS_ACCEPT] = accept;
+        scal[SC_EPS] = eps;
+        scal[SC_HNEXT] = hn;
+        scal[SC_ACCEPT] = (double)accept;
+        sg.iscal[IS_ACCEPT] = accept;
+      }
     }
   }
 }
@@ -238,7 +278,8 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
 
 }  // namespace
 
-// M = index of the current row; its time t[M] is read on the device (the RK step keeps t there).
+// M = index of the current row; its time t[M] is read on the device (the RK step keeps t there).  With
+// stage->dev_rows set, M is read on the device too and the host's M only sizes launches (pass n_cap).
 int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, const double *mu_hist,
                     const double *hist, const dmfe_rhs_out *out, const dmfe_stage *stage, double *deriv_row) {
   const int L = ctx->p.L;
@@ -269,9 +310,10 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   ps.coefT = reinterpret_cast<double4 *>(ctx->coefT);
   ps.omega = ctx->omega;
   CUDA_TRY(ctx, launch_pdl(prepare_kernel, pb, PREP_THREADS, 0, ctx->stream, L, M, ctx->model, sg, ctx->theta,
-                           ctx->nu, t, (const double4 *)hist, ctx->cur, ctx->rowtab, ctx->blo, ctx->scal, ps));
-  if (stage && stage->after_prepass) CUDA_TRY(ctx, cudaEventRecord(stage->after_prepass, ctx->stream));
+                           ctx->nu, t, (const double4 *)hist, ctx->cur, ctx->rowtab, ctx->blo, ctx->scal, mu_hist,
+                           ctx->muw, ps));
   RhsArgs a;
+  memset(&a, 0, sizeof(a));
   a.L = L;
   a.M = M;
   a.theta = ctx->theta;
@@ -285,14 +327,25 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   a.cur = ctx->cur;
   a.rowtab = ctx->rowtab;
   a.blo = ctx->blo;
+  a.muw = ctx->muw;
   a.br = ctx->br;
   a.jtop = ctx->jtop;
   a.coefM = reinterpret_cast<const double4 *>(ctx->coefM);
   a.coefT = reinterpret_cast<const double4 *>(ctx->coefT);
   a.scal = ctx->scal;
   a.deriv_row = reinterpret_cast<double4 *>(deriv_row);
+  if (stage && stage->dev_rows) {
+    a.dev_rows = stage->dev_rows;
+    a.dev_status = ctx->iscal + IS_STATUS;
+    a.complete = stage->complete;
+    a.mu_w = stage->mu;
+    a.energy_w = stage->energy;
+    a.hist_w = reinterpret_cast<double4 *>(stage->hist);
+  }
   a.out = *out;
-  const bool timed = ctx->timing_on && ctx->ev_n < DMFE_EV_RING;
+  cudaStreamCaptureStatus cap_status = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(ctx->stream, &cap_status);
+  const bool timed = ctx->timing_on && ctx->ev_n < DMFE_EV_RING && cap_status == cudaStreamCaptureStatusNone;
   if (timed) {
     if (ctx->ev_n >= ctx->ev_made) {
       CUDA_TRY(ctx, cudaEventCreate(&ctx->ev[2 * ctx->ev_made]));
@@ -328,6 +381,6 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
     CUDA_TRY(ctx, cudaEventRecord(ctx->ev[2 * ctx->ev_n + 1], ctx->stream));
     ctx->ev_n++;
   }
-  CUDA_TRY(ctx, cudaGetLastError());
+  if (cap_status == cudaStreamCaptureStatusNone) CUDA_TRY(ctx, cudaGetLastError());
   return DMFE_OK;
 }

@@ -64,7 +64,8 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
   extern __shared__ double4 smem_dyn[];
   pdl_launch_dependents();
   pdl_wait();
-  const int L = a.L, M = a.M;
+  if (batch_stopped(a)) return;
+  const int L = a.L, M = current_row(a);
   const double2 *cur = a.cur;
   const double2 *rowtab = a.rowtab;
   const int32_t *blo = a.blo;
@@ -268,7 +269,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
     else
       __syncwarp();
     if (tig == 0)
-      combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur);
+      combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur, M);
   }
 }
 

@@ -70,7 +70,8 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
   extern __shared__ double4 smem_dyn[];
   pdl_launch_dependents();
   pdl_wait();
-  const int L = a.L, M = a.M;
+  if (batch_stopped(a)) return;
+  const int L = a.L, M = current_row(a);
   const double2 *cur = a.cur;
   const double2 *rowtab = a.rowtab;
   const int2 *br = a.br;
@@ -180,6 +181,26 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
         if (lane == 0) red[parity][warp][slot[q]] = v;
       }
     };
+    // the first table entries of the type-2 half are requested before the type-1 loop starts, so
+    // that the second loop does not begin with a round trip to memory (matters for small L, where
+    // a thread has only a few pairs)
+    const int jt = a.jtop[i];
+    const uint64_t *pt2 = a.tab + plane + (size_t)i * (size_t)L + tig;  // phi2 entry of pair k
+    const uint64_t *pt3 = pt2 + plane;                                   // psi entry of pair k
+    const double2 *pn = a.thnu + tig;                                    // {theta_j, nu_j}
+    // entries of pairs k (c) and k + 1 (n); the loops request those of pair k + 2
+    uint64_t e2_c = 0, e3_c = 0, e2_n = 0, e3_n = 0;
+    double2 tn_c = make_double2(0.0, 0.0), tn_n = tn_c;
+    if (K > 0) {
+      e2_c = ld_stream(pt2);
+      e3_c = ld_stream(pt3);
+      tn_c = *pn;
+    }
+    if (K > 1) {
+      e2_n = ld_stream(pt2 + TG);
+      e3_n = ld_stream(pt3 + TG);
+      tn_n = pn[TG];
+    }
     if (top1)
       type1(std::true_type{});
     else
@@ -188,12 +209,8 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
     // ================= type-2 half: S2, S4, S7, S8 =================
     {
       double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
-      const int jt = a.jtop[i];
       int Kg = (jt > tig) ? (jt - tig + TG - 1) / TG : 0;  // this thread's pairs with j < jtop[i]
       if (Kg > K) Kg = K;
-      const uint64_t *pt2 = a.tab + plane + (size_t)i * (size_t)L + tig;  // phi2 entry of pair k
-      const uint64_t *pt3 = pt2 + plane;                                   // psi entry of pair k
-      const double2 *pn = a.thnu + tig;                                    // {theta_j, nu_j}
       auto finish = [&](double nj, double C2, double R2, double B2C, double B2R) {
         const double nR2 = nj * R2;
         const double K2 = f2<PD>(mc, C2) * nR2;
@@ -202,19 +219,6 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
         acc2 = fma(f1<PD>(mc, B2C), nR2, acc2);        // S7: D(s,t') R(t,s)
         acc3 = fma(nR2, f2<PD>(mc, B2C) * B2R, acc3);  // S8: R(t,s) K(s,t')
       };
-      // entries of pairs k (c) and k + 1 (n); the loops request those of pair k + 2
-      uint64_t e2_c = 0, e3_c = 0, e2_n = 0, e3_n = 0;
-      double2 tn_c = make_double2(0.0, 0.0), tn_n = tn_c;
-      if (K > 0) {
-        e2_c = ld_stream(pt2);
-        e3_c = ld_stream(pt3);
-        tn_c = *pn;
-      }
-      if (K > 1) {
-        e2_n = ld_stream(pt2 + TG);
-        e3_n = ld_stream(pt3 + TG);
-        tn_n = pn[TG];
-      }
       int k = 0;
       // ---- general pairs (j < jtop[i]: n2 <= M-2, both rows complete): row search, theta-stencil
       // on the cells of rows n2 and n2 + 1, cubic Hermite in t.  Index stage (the integer half of
@@ -353,7 +357,7 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
         if (!top1) hi = hist[(size_t)(n1 + 1) * (size_t)L];
         b1c_first = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
       }
-      combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur);
+      combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur, M);
     }
   }
 }

@@ -199,6 +199,7 @@ struct RhsArgs {
   const double2 *cur;     // [L] {C, R} of row M
   const double2 *rowtab;  // [M] {t_n, 1/(t_{n+1} - t_n)}
   const int32_t *blo;     // [L] blo[c] = n(theta_c t_M)
+  const double2 *muw;     // [L] mu(theta_c t_M) = muw.x + muw.y mu(t_M)  (reading G11)
   const int2 *br;         // [L-3] S = 4: row bracket of the grid cell of phi2, indexed by the stencil start
   const int32_t *jtop;    // [L]   S = 4: first node j of target i whose type-2 interval is the top one
   const double4 *coefM;   // [L-3][2] S = 4: centred cubics of {C, R} of row M per stencil start
@@ -206,17 +207,28 @@ struct RhsArgs {
   const double *scal;     // SC_MU, SC_E written by prepare_kernel
   int32_t G;              // warps per target group
   double4 *deriv_row;     // optional: row of the history whose derivative slots receive F
+  // device-resident step (rk_step.cu): M is read from dev_rows[0]; when `complete` is set the
+  // evaluation completes the appended row M: mu_w[M], energy_w[M] and the derivative slots of hist_w[M]
+  const int32_t *dev_rows;
+  const int32_t *dev_status;
+  int32_t complete;
+  double *mu_w, *energy_w;
+  double4 *hist_w;
   dmfe_rhs_out out;
 };
 
+// current row of a launch: the host's value or, in a device-resident step, the device's
+__device__ __forceinline__ int current_row(const RhsArgs &a) { return a.dev_rows ? a.dev_rows[0] : a.M; }
+__device__ __forceinline__ bool batch_stopped(const RhsArgs &a) { return a.dev_status && a.dev_status[0] != 0; }
+
 // Reduction over j of a group's eight sums and the O(1) work per target: Eq.(1), the
-// second-argument equations (readings G9, G10), mu(theta_i t) (G11) and the ray derivative of
+// second-argument equations (readings G9, G10) and the ray derivative of
 // Eq.(22).  red[warp][k] holds the warp sums; called by the group's first thread after the barrier.
 template <int PD, bool SMT>
 __device__ __forceinline__ void combine_target(const RhsArgs &a, const ModelCoef &mc, int i, int n1, double th_i,
                                                double om_i, double tM, double tau1, double b1c_first,
-                                               const double (*red)[8], int w0, int G, const double2 *cur) {
-  const int L = a.L, M = a.M;
+                                               const double (*red)[8], int w0, int G, const double2 *cur, int M) {
+  const int L = a.L;
   double Sd[8];
 #pragma unroll
   for (int k = 0; k < 8; ++k) {
@@ -227,19 +239,10 @@ __device__ __forceinline__ void combine_target(const RhsArgs &a, const ModelCoef
   }
   if (a.out.rows1) a.out.rows1[i] = n1;
   const double mu = a.scal[SC_MU];
-  // mu(theta_i t): local 4-point Lagrange in t over rows k..k+3 (reading G11), mu_M = mu
-  const int npts = (M + 1 < 4) ? M + 1 : 4;
-  int k0 = n1 - 1;
-  if (k0 > M + 1 - npts) k0 = M + 1 - npts;
-  if (k0 < 0) k0 = 0;
-  double mu_p = 0.0;
-  for (int p = 0; p < npts; ++p) {
-    double wgt = 1.0;
-    for (int q = 0; q < npts; ++q)
-      if (q != p) wgt *= (tau1 - a.t[k0 + q]) / (a.t[k0 + p] - a.t[k0 + q]);
-    const double mv = (k0 + p == M) ? mu : a.mu_hist[k0 + p];
-    mu_p += wgt * mv;
-  }
+  // mu(theta_i t): local 4-point Lagrange in t (reading G11); the pre-pass formed the part that comes
+  // from the stored rows and the weight of the current row's mu
+  const double2 mw = a.muw[i];
+  const double mu_p = fma(mw.y, mu, mw.x);
   const double2 ci = SMT ? cur[i] : a.cur[i], c0 = SMT ? cur[0] : a.cur[0];
   const double fc = mc.beta0 * f1<PD>(mc, c0.x) * b1c_first;
   const double fc2 = mc.beta0 * f1<PD>(mc, b1c_first) * c0.x;
@@ -256,14 +259,19 @@ __device__ __forceinline__ void combine_target(const RhsArgs &a, const ModelCoef
     a.out.F[2 * i] = FC;
     a.out.F[2 * i + 1] = FR;
   }
-  if (a.deriv_row) {  // the ray derivative is stored with the appended row
-    double *cell = reinterpret_cast<double *>(a.deriv_row + i);
+  double4 *drow = a.complete ? a.hist_w + (size_t)M * (size_t)L : a.deriv_row;
+  if (drow) {  // the ray derivative is stored with the appended row
+    double *cell = reinterpret_cast<double *>(drow + i);
     cell[1] = FC;
     cell[3] = FR;
   }
   if (i == 0) {
     if (a.out.mu) a.out.mu[0] = mu;
     if (a.out.energy) a.out.energy[0] = a.scal[SC_E];
+    if (a.complete) {
+      a.mu_w[M] = mu;
+      if (a.energy_w) a.energy_w[M] = a.scal[SC_E];
+    }
   }
 }
 

@@ -19,7 +19,7 @@ DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE
 
 EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror", "dmfe_get_tables",
            "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_init_state", "dmfe_rk_step",
-           "dmfe_dp_step", "dmfe_set_step_size",
+           "dmfe_advance", "dmfe_dp_step", "dmfe_set_step_size",
            "dmfe_sparsify", "dmfe_set_sparsify_threshold", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
            "dmfe_probe_fp64_tflops"]
 
@@ -42,6 +42,11 @@ class dmfe_rhs_out(Structure):
 class dmfe_state(Structure):
     _fields_ = [("n_rows", c_int32), ("n_cap", c_int32), ("t", c_void_p), ("mu", c_void_p), ("energy", c_void_p),
                 ("hist", c_void_p), ("h", c_double), ("eps_rk", c_double), ("n_rhs", c_int64)]
+
+
+class dmfe_advance_result(Structure):
+    _fields_ = [("steps", c_int32), ("accepted", c_int32), ("reverted", c_int32), ("n_rows", c_int32),
+                ("last_accepted", c_int32), ("t_last", c_double), ("h_next", c_double), ("eps_rk", c_double)]
 
 
 class DmfeError(RuntimeError):
@@ -80,6 +85,9 @@ def load_library():
     lib.dmfe_init_state.argtypes = [c_void_p, POINTER(dmfe_state), c_double]
     lib.dmfe_rk_step.restype = c_int
     lib.dmfe_rk_step.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32)]
+    lib.dmfe_advance.restype = c_int
+    lib.dmfe_advance.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, c_int32, POINTER(dmfe_advance_result),
+                                 c_void_p]
     lib.dmfe_dp_step.restype = c_int
     lib.dmfe_dp_step.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32)]
     lib.dmfe_set_step_size.restype = c_int
@@ -201,6 +209,18 @@ def dmfe_rk_step(ctx, st, fixed_step=False):
     acc = c_int32(0)
     _check(load_library().dmfe_rk_step(ctx, byref(st), 1 if fixed_step else 0, byref(acc)), "dmfe_rk_step", ctx)
     return bool(acc.value)
+
+
+def dmfe_advance(ctx, st, n_steps, fixed_step=False, want_log=False, check=True):
+    """n_steps device-resident SSPRK(10,4) steps (one CUDA graph launch per step, one record back per
+    batch).  -> (dmfe_advance_result, log[steps, 4] or None, return code).  With check=True a stop code
+    (minimal step, non-finite error) raises DmfeError; capacity always does."""
+    res = dmfe_advance_result()
+    log = np.zeros((n_steps, 4)) if want_log else None
+    rc = load_library().dmfe_advance(ctx, byref(st), int(n_steps), 1 if fixed_step else 0, byref(res), _host(log))
+    if rc != DMFE_OK and (check or rc in (DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY)):
+        _check(rc, "dmfe_advance", ctx)
+    return res, (log[:res.steps] if want_log else None), rc
 
 
 def dmfe_dp_step(ctx, st, fixed_step=False):
