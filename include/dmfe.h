@@ -122,6 +122,8 @@ typedef struct {
   double h;        /* current step size (host copy; the device copy lives in the context)        */
   double eps_rk;   /* Eq.(25) of the last attempted step (host copy)                              */
   int64_t n_rhs;   /* history-integral evaluations so far                                         */
+  int32_t acc_since; /* dmfe_integrate: steps accepted since the history was last thinned          */
+  int32_t startup;   /* dmfe_integrate: 1 while the run is in its Dormand-Prince start-up          */
 } dmfe_state;
 
 /* Row 0 at t = 0 (G13): C = R = 1, ray slopes -T(1-theta), -mu0(1-theta), mu0 = T + beta0 f'(1);
@@ -177,11 +179,52 @@ DMFE_API int dmfe_set_step_size(dmfe_ctx *ctx, dmfe_state *st, double h);
 DMFE_API int dmfe_sparsify(dmfe_ctx *ctx, dmfe_state *st, int32_t protect_last, int32_t *n_rows_out,
                   uint8_t *keep_mask);
 
-/* Threshold that eps_sparse of Eq.(27) is compared with.  The paper fixes it at tol/10
- * (PAPER.md:334), which is the default (eps_sparse = 0 restores it).  A caller that must keep the
- * history below a hard row cap (BASELINE.json configs 3, 4) raises it when a forced pass frees too
- * little (reading G25 in DESIGN.md); every such change is the caller's and is reported by it. */
-DMFE_API int dmfe_set_sparsify_threshold(dmfe_ctx *ctx, double eps_sparse);
+/* The step loop of a run: when to thin the history, how many greedy passes a
+ * thinning takes (PAPER.md:336 makes "the number of sparsification passes" a user control), the
+ * Dormand-Prince start-up and its switch to SSPRK(10,4).  The paper fixes none of the
+ * numbers below except the Eq.(27) threshold tol/10, which is NOT a parameter here (reading G25).
+ * A zero field selects the default in brackets. */
+typedef struct {
+  int32_t batch;         /* SSPRK(10,4) steps per device batch; the loop below looks at the state only
+                            between batches [50]                                                      */
+  int32_t sp_every;      /* thin the history once this many steps were accepted since the last time
+                            [200]                                                                     */
+  int32_t sp_max_passes; /* greedy passes per thinning at most [8] ...                                */
+  double sp_min_gain;    /* ... repeated while a pass still drops this fraction of the rows [0.01]    */
+  int32_t protect_last;  /* newest rows that are never dropped: two consecutive reverts take back 20
+                            rows [24]                                                  */
+  int32_t startup_dp;    /* != 0: start with Dormand-Prince steps and switch to SSPRK(10,4) with
+                            min(h/2, Eq.(24) cap) when h 4 sqrt(f''(1)) >= 3.3 (reading G21) [0]      */
+} dmfe_policy;
+
+typedef struct {
+  int64_t steps;           /* attempted steps ...                                                     */
+  int64_t accepted;        /* ... of which accepted ...                                               */
+  int64_t reverted;        /* ... and reverted                                                        */
+  int64_t dp_steps;        /* Dormand-Prince steps among them                                         */
+  int64_t sparsify_calls;  /* thinnings ...                                                           */
+  int64_t sparsify_passes; /* ... greedy passes they took ...                                         */
+  int64_t rows_dropped;    /* ... rows they dropped                                                   */
+  int32_t n_rows;          /* complete rows now                                                       */
+  int32_t n_rows_max;      /* most rows held at any time                                              */
+  int32_t status;          /* DMFE_OK or the code that ended the loop                                 */
+  int32_t pad;
+  double t;                /* time of the last complete row                                           */
+  double h;                /* next step size                                                          */
+  double eps_rk;           /* Eq.(25) of the last step                                                */
+} dmfe_run_stats;
+
+/* Runs the step loop until t >= t_end, max_steps more steps were attempted (<= 0: no limit) or
+ * max_seconds of wall time have passed (<= 0: no limit); stats (in/out) accumulates over calls:
+ *   loop:  thin the history if due (acc_since >= sp_every, or fewer than two free rows): passes of
+ *          dmfe_sparsify until one drops less than sp_min_gain of the rows or sp_max_passes is reached;
+ *          still fewer than two free rows: DMFE_ECAPACITY;
+ *          start-up: h 4 sqrt(f''(1)) >= 3.3 -> h = min(h/2, cap) and SSPRK(10,4) from then on, else one
+ *          dmfe_dp_step; otherwise dmfe_advance(min(batch, steps left)).
+ * The test oracle holds the same loop; the tests compare the two decision for decision.
+ * st->acc_since and st->startup carry the loop's state between calls. */
+DMFE_API int dmfe_integrate(dmfe_ctx *ctx, dmfe_state *st, const dmfe_policy *policy, double t_end,
+                            int64_t max_steps, double max_seconds, dmfe_run_stats *stats);
 
 /* Measurement hooks (bench.py).  dmfe_enable_timing: when on, every dmfe_history_integrals launch
  * records CUDA events on the context's stream immediately before and after the pair kernel (the

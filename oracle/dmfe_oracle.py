@@ -522,3 +522,91 @@ def run_adaptive(grid: Grid, model: Model, t_end: float, tol: float, h0=1e-3, n_
         if h < h_min:
             raise RuntimeError("step below h_min")
     return H
+
+
+# --------------------------------------------------------------------------- the step loop of a run
+@dataclass
+class Policy:
+    """The loop's free parameters (PAPER.md:334-336 leaves the thinning schedule and the number of passes to
+    the user, PAPER.md:316 the start-up switch; reading G25/G21).  The Eq.(27) threshold tol/10 is not one."""
+    batch: int = 50            # SSPRK steps between two looks at the state
+    sp_every: int = 200        # thin the history once this many steps were accepted since the last time
+    sp_max_passes: int = 8     # greedy passes per thinning at most ...
+    sp_min_gain: float = 0.01  # ... repeated while a pass still drops this fraction of the rows
+    protect_last: int = 24     # two consecutive reverts take back 20 rows (PAPER.md:320)
+    startup_dp: bool = False
+
+
+@dataclass
+class RunState:
+    h: float
+    acc_since: int = 0
+    startup: bool = False
+    status: str = "ok"
+    log: list = field(default_factory=list)   # (accepted, eps_RK, h_next, n_rows) per attempted step
+    masks: list = field(default_factory=list)  # keep mask of every thinning pass
+
+
+def integrate(H: History, policy: Policy, rs: RunState, t_end: float, tol: float, max_steps: int = 0,
+              h_min: float = 1e-12):
+    """The step loop of a run, as the library's dmfe_integrate holds it:
+      loop until t >= t_end (or max_steps more steps):
+        thin the history if due (acc_since >= sp_every, or fewer than two free rows): greedy passes
+          (PAPER.md:334) until one drops less than sp_min_gain of the rows or sp_max_passes is reached;
+          still fewer than two free rows: capacity error;
+        start-up (PAPER.md:316): h 4 sqrt(f''(1)) >= 3.3 -> h = min(h/2, cap), SSPRK(10,4) from then on;
+          else one Dormand-Prince step;
+        otherwise min(batch, steps left, free rows) SSPRK(10,4) steps with the controller of PAPER.md:320;
+          a step that leaves h < h_min ends the run.
+    Returns the number of steps attempted in this call."""
+    model = H.model
+    if H.n_rows == 1 and policy.startup_dp:
+        rs.startup = True
+    done = 0
+    while H.t[H.n_rows - 1] < t_end:
+        if max_steps > 0 and done >= max_steps:
+            break
+        if rs.acc_since >= policy.sp_every or H.n_rows + 2 > H.n_cap:
+            for _ in range(policy.sp_max_passes):
+                before = H.n_rows
+                keep, _eps = sparsify(H, tol, policy.protect_last)
+                rs.masks.append(keep)
+                freed = before - H.n_rows
+                if freed < policy.sp_min_gain * before or freed < 1:
+                    break
+            rs.acc_since = 0
+            if H.n_rows + 2 > H.n_cap:
+                rs.status = "capacity"
+                break
+        if rs.startup:
+            if dp_must_switch(model, rs.h):
+                rs.startup = False
+                rs.h = min(rs.h / 2.0, h_stab(model))
+                continue
+            ok, rs.h, eps = dp_controller_step(H, rs.h, tol)
+            rs.log.append((ok, eps, rs.h, H.n_rows))
+            done += 1
+            if ok:
+                rs.acc_since += 1
+            if rs.h < h_min:
+                rs.status = "stepmin"
+                break
+        else:
+            nb = policy.batch
+            if max_steps > 0:
+                nb = min(nb, max_steps - done)
+            nb = min(nb, H.n_cap - H.n_rows)
+            stop = False
+            for _ in range(nb):
+                ok, rs.h, eps = controller_step(H, rs.h, tol)
+                rs.log.append((ok, eps, rs.h, H.n_rows))
+                done += 1
+                if ok:
+                    rs.acc_since += 1
+                if rs.h < h_min:
+                    rs.status = "stepmin"
+                    stop = True
+                    break
+            if stop:
+                break
+    return done

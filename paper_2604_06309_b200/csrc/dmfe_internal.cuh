@@ -54,7 +54,6 @@ struct dmfe_ctx {
   int sm_count;  // SMs of the device the context was created on
   int smem_max;  // opt-in dynamic shared memory per CTA, minus the kernels' static use
   double gamma, A, B;  // gamma = -W_{-1}(-1/t_max); A = atan(e^gamma), B = atan(e^-gamma)
-  double eps_sparse;   // threshold of Eq.(27); 0 = the paper's tol/10
   double h_stab;       // 13.9 / (4 sqrt(f''(1)))  (Eq.(24))
   // ---- tables (device) ----
   double *theta, *omega, *nu;  // [L]

@@ -126,6 +126,8 @@ int dmfe_init_state(dmfe_ctx *ctx, dmfe_state *st, double h0) {
   st->h = h;
   st->eps_rk = 0.0;
   st->n_rhs = 0;
+  st->acc_since = 0;
+  st->startup = 0;
   return DMFE_OK;
 }
 

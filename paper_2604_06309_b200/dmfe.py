@@ -20,7 +20,7 @@ DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE
 EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror", "dmfe_get_tables",
            "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_init_state", "dmfe_rk_step",
            "dmfe_advance", "dmfe_dp_step", "dmfe_set_step_size",
-           "dmfe_sparsify", "dmfe_set_sparsify_threshold", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
+           "dmfe_sparsify", "dmfe_integrate", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
            "dmfe_probe_fp64_tflops"]
 
 
@@ -41,7 +41,20 @@ class dmfe_rhs_out(Structure):
 
 class dmfe_state(Structure):
     _fields_ = [("n_rows", c_int32), ("n_cap", c_int32), ("t", c_void_p), ("mu", c_void_p), ("energy", c_void_p),
-                ("hist", c_void_p), ("h", c_double), ("eps_rk", c_double), ("n_rhs", c_int64)]
+                ("hist", c_void_p), ("h", c_double), ("eps_rk", c_double), ("n_rhs", c_int64),
+                ("acc_since", c_int32), ("startup", c_int32)]
+
+
+class dmfe_policy(Structure):
+    _fields_ = [("batch", c_int32), ("sp_every", c_int32), ("sp_max_passes", c_int32), ("sp_min_gain", c_double),
+                ("protect_last", c_int32), ("startup_dp", c_int32)]
+
+
+class dmfe_run_stats(Structure):
+    _fields_ = [("steps", c_int64), ("accepted", c_int64), ("reverted", c_int64), ("dp_steps", c_int64),
+                ("sparsify_calls", c_int64), ("sparsify_passes", c_int64), ("rows_dropped", c_int64),
+                ("n_rows", c_int32), ("n_rows_max", c_int32), ("status", c_int32), ("pad", c_int32),
+                ("t", c_double), ("h", c_double), ("eps_rk", c_double)]
 
 
 class dmfe_advance_result(Structure):
@@ -94,8 +107,9 @@ def load_library():
     lib.dmfe_set_step_size.argtypes = [c_void_p, POINTER(dmfe_state), c_double]
     lib.dmfe_sparsify.restype = c_int
     lib.dmfe_sparsify.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32), c_void_p]
-    lib.dmfe_set_sparsify_threshold.restype = c_int
-    lib.dmfe_set_sparsify_threshold.argtypes = [c_void_p, c_double]
+    lib.dmfe_integrate.restype = c_int
+    lib.dmfe_integrate.argtypes = [c_void_p, POINTER(dmfe_state), POINTER(dmfe_policy), c_double, c_int64, c_double,
+                                   POINTER(dmfe_run_stats)]
     lib.dmfe_enable_timing.restype = c_int
     lib.dmfe_enable_timing.argtypes = [c_void_p, c_int32]
     lib.dmfe_last_kernel_ms.restype = c_int
@@ -196,7 +210,7 @@ def make_state(L, n_cap, device="cuda"):
                energy=torch.zeros(n_cap, dtype=torch.float64, device=device),
                hist=torch.zeros((n_cap, L, 4), dtype=torch.float64, device=device))
     st = dmfe_state(n_rows=0, n_cap=n_cap, t=_dev(ten["t"]), mu=_dev(ten["mu"]), energy=_dev(ten["energy"]),
-                    hist=_dev(ten["hist"]), h=0.0, eps_rk=0.0, n_rhs=0)
+                    hist=_dev(ten["hist"]), h=0.0, eps_rk=0.0, n_rhs=0, acc_since=0, startup=0)
     return st, ten
 
 
@@ -242,8 +256,16 @@ def dmfe_sparsify(ctx, st, protect_last=12, want_mask=False):
     return n_out.value, (mask.astype(bool) if want_mask else None)
 
 
-def dmfe_set_sparsify_threshold(ctx, eps_sparse):
-    _check(load_library().dmfe_set_sparsify_threshold(ctx, float(eps_sparse)), "dmfe_set_sparsify_threshold", ctx)
+def dmfe_integrate(ctx, st, policy, t_end, max_steps=0, max_seconds=0.0, stats=None, check=True):
+    """The step loop of a run inside the library (thinning schedule, start-up switch, batches of steps).
+    -> (stats, return code); stats accumulates over calls when passed back in."""
+    if stats is None:
+        stats = dmfe_run_stats()
+    rc = load_library().dmfe_integrate(ctx, byref(st), byref(policy) if policy is not None else None, float(t_end),
+                                       int(max_steps), float(max_seconds), byref(stats))
+    if rc != DMFE_OK and check:
+        _check(rc, "dmfe_integrate", ctx)
+    return stats, rc
 
 
 def dmfe_enable_timing(ctx, on=True):

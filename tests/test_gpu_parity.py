@@ -206,6 +206,33 @@ def test_rhs_mode1_row_table_in_global_memory_sampled_targets(D):
     _sampled_blocks_parity(D, 8192, 4, 1e7, [0, 0, 1.0, 0.8, 0.5], -2.0, 7.0, n_blocks=4)
 
 
+def test_rhs_one_warp_per_target_launch_shape_all_targets(D):
+    """L = 2304 = just below 16 x 148 warps: the launcher gives every target ONE warp (G = 1: no cross-warp
+    reduction, no group barrier) -- the launch shape of the L = 16384 and 32768 sweep points.  All targets,
+    row indices bit-exact."""
+    L, s, t_max, lam = 2304, 4, 1e4, [0, 0, 1.0, 0.8, 0.5]
+    ctx = D.dmfe_create(L, s, t_max, lam, T=0.5)
+    try:
+        tab = D.dmfe_get_tables(ctx, L)
+        grid = _oracle_grid_from_library(tab, L, s, t_max)
+        N = 700
+        t, mu, hist = inputs.synthetic_history(tab["theta"], tab["omega"], N, -2.0, 4.0)
+        g = gpu_rhs(D, ctx, L, t, mu, hist, N)
+    finally:
+        D.dmfe_destroy(ctx)
+    model = O.Model(np.array(lam, dtype=np.float64), 0.5, 0.0)
+    ref = O.history_integrals(grid, model, t, mu, hist, N - 1, tables=(tab["start"], tab["frac"]), want_rows=True)
+    ref["theta"] = tab["theta"]
+    compare_rhs(g, ref)
+
+
+def test_rhs_config5_L16384_sampled_targets(D):
+    """BASELINE.json configs[4] at L = N = 16384 (8.6 GB of history, 6.4 GB of pair tables, one warp per
+    target, per-call tables in global memory): 512 seeded targets (16 blocks of 32, first and last included)
+    against the oracle, as SURVEY.md 8(d) asks for L >= 16384."""
+    _sampled_blocks_parity(D, 16384, 4, 1e7, [0, 0, 1.0, 0.8, 0.5], -2.0, 7.0, n_blocks=14)
+
+
 def test_rhs_closed_form_constant_history_full_size_all_targets(D):
     """A property that holds at any size, checked on every target of the bench-size evaluation
     (L = N = 4096, log-spaced rows of config 2) without the oracle: for the constant history

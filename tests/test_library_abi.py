@@ -52,10 +52,21 @@ def _header_struct_fields(name):
     return fields
 
 
-@pytest.mark.parametrize("name", ["dmfe_params", "dmfe_grid", "dmfe_rhs_out", "dmfe_state"])
+@pytest.mark.parametrize("name", ["dmfe_params", "dmfe_grid", "dmfe_rhs_out", "dmfe_state", "dmfe_advance_result",
+                                  "dmfe_policy", "dmfe_run_stats"])
 def test_struct_field_order_matches_header(name):
     from paper_2604_06309_b200 import dmfe
     assert [f[0] for f in getattr(dmfe, name)._fields_] == _header_struct_fields(name)
+
+
+def test_struct_sizes_match_the_c_layout():
+    """ctypes lays the mirrored structs out like the C compiler does (natural alignment)."""
+    import ctypes
+    from paper_2604_06309_b200 import dmfe
+    assert ctypes.sizeof(dmfe.dmfe_advance_result) == 5 * 4 + 4 + 3 * 8
+    assert ctypes.sizeof(dmfe.dmfe_policy) == 3 * 4 + 4 + 8 + 2 * 4
+    assert ctypes.sizeof(dmfe.dmfe_run_stats) == 7 * 8 + 4 * 4 + 3 * 8
+    assert dmfe.dmfe_policy.sp_min_gain.offset == 16 and dmfe.dmfe_policy.protect_last.offset == 24
 
 
 def test_product_does_not_import_the_oracle():

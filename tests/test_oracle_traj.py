@@ -361,3 +361,56 @@ def test_controller_constants_from_a_stubbed_error_sequence(monkeypatch):
     # the cap of Eq.(24)
     ok, h2, _ = (lambda: (monkeypatch.setattr(O, "rk_step", lambda H_, h_: 0.0), O.controller_step(H, cap, tol))[1])()
     assert ok and h2 == cap
+
+
+# ------------------------------------------------------------------------------------ step loop
+def test_greedy_walk_equals_odd_positions_of_flagged_runs():
+    """PAPER.md:334 "drop n, then skip to n+2": a candidate's neighbours are never removed before it is
+    tested, so the sequential walk equals "in every maximal run of flagged candidates drop the 1st, 3rd,
+    5th ..." (the form a parallel implementation can use).  Random flag patterns, brute force."""
+    rng = np.random.default_rng(7)
+    for trial in range(200):
+        N = int(rng.integers(3, 60))
+        protect = int(rng.integers(0, 8))
+        eps = np.where(rng.random(N) < rng.uniform(0.2, 0.9), 0.0, 1.0)
+        eps[0] = eps[-1] = np.inf
+        keep = O.sparsify_mask(eps, N, tol=1.0, protect_last=protect)
+        exp = np.ones(N, dtype=bool)
+        last = min(N - 1 - protect, N - 2)
+        run = 0
+        for n in range(1, N):
+            flagged = n <= last and eps[n] < 0.1
+            run = run + 1 if flagged else 0
+            if flagged and run % 2 == 1:
+                exp[n] = False
+        assert np.array_equal(keep, exp)
+
+
+@pytest.mark.slow
+def test_step_loop_thinning_passes_and_startup():
+    """The oracle's step loop (integrate): Dormand-Prince start-up switches once, periodic thinning with
+    several greedy passes drops more rows than one pass, constraints are kept, the state is resumable
+    (two calls = one call), and a cap the rule cannot hold ends the run with the capacity status."""
+    grid = O.Grid(L=32, s=4, t_max=100.0)
+    model = O.Model(lam=[0.0, 0.0, 0.0, 1.0], T=0.5)
+    tol = 1e-3          # loose: the step keeps growing by 1.01 and reaches the start-up switch after ~620 steps
+
+    def run(passes, chunks, n_cap=300):
+        H = O.History(grid, model, n_cap)
+        rs = O.RunState(h=1e-3)
+        pol = O.Policy(batch=8, sp_every=40, sp_max_passes=passes, protect_last=24, startup_dp=True)
+        for n in chunks:
+            O.integrate(H, pol, rs, 1e300, tol, max_steps=n)
+        return H, rs
+
+    H1, r1 = run(1, [700])
+    H4, r4 = run(4, [700])
+    assert r1.status == r4.status == "ok" and not r4.startup
+    assert H4.n_rows < H1.n_rows and len(r4.masks) > len(r1.masks)
+    n = H4.n_rows
+    assert np.abs(H4.hist[:n, -1, 0] - 1.0).max() < 1e-12 and np.abs(H4.hist[:n, -1, 2] - 1.0).max() < 1e-12
+    # resumable: the same 700 steps in three calls whose boundaries coincide with batch boundaries
+    Hc, rc_ = run(4, [8 * 11, 8 * 30, 700 - 8 * 41])
+    assert Hc.n_rows == H4.n_rows and rc_.h == r4.h and np.array_equal(Hc.t[:n], H4.t[:n])
+    Ht, rt = run(4, [700], n_cap=40)
+    assert rt.status == "capacity" and Ht.n_rows + 2 > 40
