@@ -386,6 +386,11 @@ def run_ours(args):
     else:
         roof = {"bound": "alu", "achieved": pairs * fpp / (k_avg_ms * 1e-3) / 1e12, "peak": fp64_tf, "unit": "TFLOP/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
+    # the same fraction with SURVEY.md 8(d)'s count of the method's own work, 24 s + 106 flop per pair
+    # (interpolation weights given, as the paper tabulates them); `flops_per_pair` above adds the
+    # recomputation of the weights from the packed coordinate, a design choice of this library
+    fpp_survey = 24 * s + 106
+    t_alu_survey = pairs * fpp_survey / (fp64_tf * 1e12)
     traffic, traffic_src = args.traffic_bytes, "--traffic-bytes"
     if traffic is None:
         try:   # dram bytes per launch of this kernel on this workload from the committed ncu capture
@@ -397,13 +402,19 @@ def run_ours(args):
             traffic, traffic_src = None, None
     roof.update({
         "traffic": traffic, "traffic_source": traffic_src, "peak_source": "hbm: %s copy bandwidth; alu: DFMA chain measured in this run "
-        "on %d SMs" % (hbm_src, sms), "kernel": "history_integrals_kernel<%d>" % s, "kernel_ms_avg": k_avg_ms,
+        "on %d SMs" % (hbm_src, sms), "kernel": ("history_integrals_s4_kernel" if s == 4 else "history_integrals_kernel<%d>" % s),
+        "kernel_ms_avg": k_avg_ms,
         "kernel_ms_min": k_min, "launches_timed": n_k, "algorithmic_bytes": alg_bytes,
         "algorithmic_bytes_sampled": sampled, "table_bytes": table_bytes, "flops_per_pair": fpp,
         "hbm": {"achieved_GBps": alg_bytes / (k_avg_ms * 1e-3) / 1e9, "peak_GBps": hbm_peak,
                 "with_tables_GBps": (alg_bytes + table_bytes) / (k_avg_ms * 1e-3) / 1e9},
         "alu": {"achieved_TFLOPs": pairs * fpp / (k_avg_ms * 1e-3) / 1e12, "peak_TFLOPs": fp64_tf},
         "roofline_time_ms": 1e3 * max(t_hbm, t_alu),
+        "survey_count": {"flops_per_pair": fpp_survey, "roofline_time_ms": 1e3 * max(t_hbm, t_alu_survey),
+                         "frac": max(t_hbm, t_alu_survey) / (k_avg_ms * 1e-3)},
+        # what this design must move through HBM per launch (history cells once per loop that touches
+        # them + the 24 B/pair tables) against the measured copy bandwidth
+        "design_bytes_hbm_frac": ((traffic if traffic else alg_bytes + table_bytes) / (hbm_peak * 1e9)) / (k_avg_ms * 1e-3),
     })
 
     # ---- the oracle on this box's host cores, bounded sample -----------------------------------
@@ -425,7 +436,10 @@ def run_ours(args):
                             "wall time" % (cfg["L"], cfg["s"], cfg["n_cap"], args.traj_seconds),
                 "steps_per_s": stt["steps"] / stt["wall_s"], "rhs_per_s": stt["n_rhs"] / stt["wall_s"],
                 "t_reached": stt["t_reached"], "wall_s_to_t": out["wall_to_t"], "reverted": stt["reverted"],
-                "n_rows": stt["n_rows"], "status": stt["status"],
+                "n_rows": stt["n_rows"], "n_rows_max": stt["n_rows_max"], "status": stt["status"],
+                "sparsify_passes": stt["sparsify_passes"], "rows_dropped": stt["rows_dropped"],
+                "eps_sparse_over_tol": stt["eps_sparse_over_tol"],
+                "us_per_stage": 1e5 * stt["wall_s"] / max(stt["steps"], 1),
                 "full_runs": "profiles/ holds the wall times of the runs to t=1e5 (config 3) and t=1e7 (config 4)"}
 
     value = job_value(EVALS_PER_PAIR * pairs, args.steps, world, ms_total)

@@ -51,7 +51,10 @@ typedef struct {
   int32_t quad_degree; /* odd degree of the global spline that defines nu_j; 5 = paper default
                           (PAPER.md:278); 1 and 3 are accepted                                   */
   int32_t p_max;       /* lambda has p_max+1 entries, 2 <= p_max <= 15                           */
-  double t_max;        /* sets gamma = -W_{-1}(-1/t_max); must be > e             */
+  double t_max;        /* sets gamma = -W_{-1}(-1/t_max); must be > e.  The grid is
+                          Eq.(16) with alpha = delta = 0 (the closed-form invertible grid): the
+                          (alpha, delta) warp of PAPER.md:217-228 is NOT offered by this library
+                          (reading G6 in DESIGN.md)                            */
   double beta0;        /* inverse temperature of the initial condition, 0 = random start (Eq.(12)) */
   double tol;          /* epsilon of Eq.(25); used by rk_step / sparsify only      */
   double h_min;        /* terminate below this step; 0 -> 1e-12                    */
