@@ -308,3 +308,159 @@ void orc_sparsify_residuals(int L, int N, const double *t, const double *hist, d
         eps_sparse[n] = (double)acc;
     }
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Values-only history ("higher-order interpolation schemes on the
+ * adaptive t grid, which would allow a further reduction of stored history points"; BASELINE.json
+ * config 2's "4-point-per-axis Lagrange stencils"): the rows hold C and R only, 16 bytes per cell,
+ * and the interpolation in t is the local 4-point Lagrange polynomial through rows k..k+3 with
+ *   k = clamp(n(tau) - 1, 0, M - 3)   (the window of orc_mu_at: one row below the interval of tau,
+ * two above, clamped at both ends; fewer rows: all of them).  The current row M is an ordinary
+ * point of the window.  Everything else is orc_history_integrals: theta-stencil first, then t
+ * (PAPER.md:266), the same eight sums, mu, E and combinations.
+ *   histv  [M+1][L][2] packed {C, R}
+ * ------------------------------------------------------------------------------------------------ */
+#define VC(n, l) histv[((size_t)(n) * (size_t)L + (size_t)(l)) * 2 + 0]
+#define VR(n, l) histv[((size_t)(n) * (size_t)L + (size_t)(l)) * 2 + 1]
+
+/* window start k, number of points and Lagrange weights in t at tau */
+int orc_t_lagrange(const double *t, int M, double tau, double *w, int *npts_out) {
+    int npts = M + 1 < 4 ? M + 1 : 4;
+    int n = orc_row_search(t, M, tau);
+    int k = n - 1;
+    if (k > M + 1 - npts) k = M + 1 - npts;
+    if (k < 0) k = 0;
+    for (int a = 0; a < npts; ++a) {
+        double wa = 1.0;
+        for (int b = 0; b < npts; ++b) {
+            if (b == a) continue;
+            wa *= (tau - t[k + b]) / (t[k + a] - t[k + b]);
+        }
+        w[a] = wa;
+    }
+    *npts_out = npts;
+    return k;
+}
+
+void orc_history_integrals_values(int L, int s, int M, const double *lam, int pmax, double T,
+                                  double beta0, const double *theta, const double *omega,
+                                  const double *nu, const double *t, const double *mu_hist,
+                                  const double *histv, int nt, const int32_t *targets,
+                                  const int32_t *start, const double *frac, double *sums,
+                                  double *abssums, double *deriv, double *scale, int32_t *rows1,
+                                  int32_t *rows2, double *mu_out, double *E_out) {
+    /* on-grid reductions, Eq.(13), Eq.(14) */
+    long double sm = 0.0L, se = 0.0L;
+    const double tM = t[M];
+    for (int j = 0; j < L; ++j) {
+        double c = VC(M, j), r = VR(M, j);
+        double fp = f1(lam, pmax, c), fpp = f2(lam, pmax, c);
+        sm += (long double)(nu[j] * (fpp * r * c + fp * r));
+        se += (long double)(nu[j] * (fp * r));
+    }
+    const double c00 = VC(M, 0);
+    const double mu = T + tM * (double)sm + beta0 * f1(lam, pmax, c00) * c00;
+    const double E = -tM * (double)se - beta0 * f0(lam, pmax, c00);
+    if (mu_out) *mu_out = mu;
+    if (E_out) *E_out = E;
+    double *mu_all = (double *)malloc(sizeof(double) * (size_t)(M + 1));
+    for (int n = 0; n < M; ++n) mu_all[n] = mu_hist[n];
+    mu_all[M] = mu;
+    const size_t plane = (size_t)nt * (size_t)L;
+
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int it = 0; it < nt; ++it) {
+        const int i = targets[it];
+        const double th_i = theta[i], om_i = omega[i];
+        long double S[8], A[8];
+        for (int k = 0; k < 8; ++k) S[k] = A[k] = 0.0L;
+        double w1[16], w2[16], w3[16], g1[4], g2[4];
+        int np1, np2;
+        /* type-1: one window per target, tau = theta_i * t  (Eq.19) */
+        const double tau1 = th_i * tM;
+        const int k1 = orc_t_lagrange(t, M, tau1, g1, &np1);
+        if (rows1) rows1[it] = k1;
+        double B1C_first = 0.0;
+        for (int j = 0; j < L; ++j) {
+            const size_t e = (size_t)it * (size_t)L + (size_t)j;
+            const int a1 = start[0 * plane + e], a2 = start[1 * plane + e], a3 = start[2 * plane + e];
+            orc_lagrange_weights(s, frac[0 * plane + e], w1);
+            orc_lagrange_weights(s, frac[1 * plane + e], w2);
+            orc_lagrange_weights(s, frac[2 * plane + e], w3);
+            double C1 = 0.0, R1 = 0.0, C2 = 0.0, R2 = 0.0;
+            for (int l = 0; l < s; ++l) {
+                C1 += w1[l] * VC(M, a1 + l);
+                R1 += w1[l] * VR(M, a1 + l);
+                C2 += w2[l] * VC(M, a2 + l);
+                R2 += w2[l] * VR(M, a2 + l);
+            }
+            /* type-1 lookup: t-interpolation of column j (Eq.19) */
+            double B1C = 0.0, B1R = 0.0;
+            for (int a = 0; a < np1; ++a) {
+                B1C += g1[a] * VC(k1 + a, j);
+                B1R += g1[a] * VR(k1 + a, j);
+            }
+            if (j == 0) B1C_first = B1C;
+            /* type-2 lookup: theta-stencil on every row of the window, then t (Eq.20) */
+            const double phi2 = th_i + om_i * theta[j];
+            const double tau2 = phi2 * tM;
+            const int k2 = orc_t_lagrange(t, M, tau2, g2, &np2);
+            if (rows2) rows2[e] = k2;
+            double B2C = 0.0, B2R = 0.0;
+            for (int a = 0; a < np2; ++a) {
+                double cr = 0.0, rr = 0.0;
+                for (int l = 0; l < s; ++l) {
+                    cr += w3[l] * VC(k2 + a, a3 + l);
+                    rr += w3[l] * VR(k2 + a, a3 + l);
+                }
+                B2C += g2[a] * cr;
+                B2R += g2[a] * rr;
+            }
+            const double nj = nu[j];
+            double term[8];
+            term[0] = nj * (f2(lam, pmax, C1) * R1 * B1C);
+            term[1] = nj * (f2(lam, pmax, C2) * R2 * B2C);
+            term[2] = nj * (f1(lam, pmax, C1) * B1R);
+            term[3] = nj * (f2(lam, pmax, C2) * R2 * B2R);
+            term[4] = nj * (f2(lam, pmax, B1C) * B1R * C1);
+            term[5] = nj * (f1(lam, pmax, B1C) * R1);
+            term[6] = nj * (f1(lam, pmax, B2C) * R2);
+            term[7] = nj * (R2 * (f2(lam, pmax, B2C) * B2R));
+            for (int k = 0; k < 8; ++k) {
+                S[k] += (long double)term[k];
+                A[k] += (long double)fabs(term[k]);
+            }
+        }
+        double Sd[8];
+        for (int k = 0; k < 8; ++k) {
+            Sd[k] = (double)S[k];
+            if (sums) sums[(size_t)it * 8 + k] = Sd[k];
+            if (abssums) abssums[(size_t)it * 8 + k] = (double)A[k];
+        }
+        if (deriv || scale) {
+            const double Ci = VC(M, i), Ri = VR(M, i), C0 = VC(M, 0);
+            const double mu_p = orc_mu_at(t, mu_all, M, tau1);
+            const double fc = beta0 * f1(lam, pmax, C0) * B1C_first;
+            const double fc2 = beta0 * f1(lam, pmax, B1C_first) * C0;
+            const double d1C = -mu * Ci + tM * (th_i * Sd[0] + om_i * Sd[1] + th_i * Sd[2]) + fc;
+            const double d1R = -mu * Ri + tM * (om_i * Sd[3]);
+            const double d2C = -mu_p * Ci + tM * (th_i * Sd[4] + th_i * Sd[5] + om_i * Sd[6]) +
+                               2.0 * T * Ri + fc2;
+            const double d2R = mu_p * Ri - tM * (om_i * Sd[7]);
+            if (deriv) {
+                double *d = deriv + (size_t)it * 6;
+                d[0] = d1C; d[1] = d1R; d[2] = d2C; d[3] = d2R;
+                d[4] = d1C + th_i * d2C;
+                d[5] = d1R + th_i * d2R;
+            }
+            if (scale) {
+                double *q = scale + (size_t)it * 4;
+                q[0] = fabs(mu * Ci) + tM * (th_i * (double)A[0] + om_i * (double)A[1] + th_i * (double)A[2]) + fabs(fc);
+                q[1] = fabs(mu * Ri) + tM * om_i * (double)A[3];
+                q[2] = fabs(mu_p * Ci) + tM * (th_i * (double)A[4] + th_i * (double)A[5] + om_i * (double)A[6]) + fabs(2.0 * T * Ri) + fabs(fc2);
+                q[3] = fabs(mu_p * Ri) + tM * om_i * (double)A[7];
+            }
+        }
+    }
+    free(mu_all);
+}

@@ -232,6 +232,43 @@ def history_integrals(grid: Grid, model: Model, t, mu_hist, hist, M: int, target
     return out
 
 
+def history_integrals_values(grid: Grid, model: Model, t, mu_hist, histv, M: int, targets=None, tables=None,
+                             want_rows=False):
+    """The same right-hand side on a VALUES-ONLY history: histv[(M+1), L, 2] =
+    {C, R}; interpolation in t = local 4-point Lagrange through rows k..k+3, k = clamp(n(tau)-1, 0, M-3).
+    rows1 / rows2 are the window starts k.  Same return dict as history_integrals."""
+    lib = _load()
+    L, s = grid.L, grid.s
+    if targets is None:
+        targets = np.arange(L)
+    targets = np.ascontiguousarray(targets, dtype=np.int32)
+    nt = len(targets)
+    if tables is None:
+        tables = grid.tables(None if nt == L and np.array_equal(targets, np.arange(L)) else targets)
+    start = np.ascontiguousarray(tables[0], dtype=np.int32)
+    frac = np.ascontiguousarray(tables[1], dtype=np.float64)
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    mu_hist = np.ascontiguousarray(mu_hist, dtype=np.float64)
+    histv = np.ascontiguousarray(histv, dtype=np.float64)
+    assert histv.ndim == 3 and histv.shape[1] == L and histv.shape[2] == 2 and histv.shape[0] >= M + 1
+    assert M >= 1 and len(t) >= M + 1 and len(mu_hist) >= M
+    sums = np.zeros((nt, 8)); abssums = np.zeros((nt, 8))
+    deriv = np.zeros((nt, 6)); scale = np.zeros((nt, 4))
+    rows1 = np.zeros(nt, dtype=np.int32) if want_rows else None
+    rows2 = np.zeros((nt, L), dtype=np.int32) if want_rows else None
+    mu = ctypes.c_double(0.0); E = ctypes.c_double(0.0)
+    lib.orc_history_integrals_values(
+        ctypes.c_int(L), ctypes.c_int(s), ctypes.c_int(M), _p(model.lam), ctypes.c_int(model.pmax),
+        ctypes.c_double(model.T), ctypes.c_double(model.beta0), _p(grid.theta), _p(grid.omega),
+        _p(grid.nu), _p(t), _p(mu_hist), _p(histv), ctypes.c_int(nt), _p(targets), _p(start),
+        _p(frac), _p(sums), _p(abssums), _p(deriv), _p(scale), _p(rows1), _p(rows2),
+        ctypes.byref(mu), ctypes.byref(E))
+    out = dict(sums=sums, abssums=abssums, deriv=deriv, scale=scale, mu=mu.value, E=E.value)
+    if want_rows:
+        out["rows1"], out["rows2"] = rows1, rows2
+    return out
+
+
 def sparsify_residuals(L: int, N: int, t, hist):
     """eps_sparse[n] of Eq.(27) for every interior row."""
     lib = _load()
