@@ -65,7 +65,7 @@ def flops_per_pair(s: int, lam) -> int:
     return 3 * (5 * s - 4) + 8 * s + 14 + 16 * s + 14 + 20 + horner + 30
 
 
-def unique_cells(theta, omega, t, s, L, N, sample=None):
+def unique_cells(theta, omega, t, s, L, N, sample=None, window=2):
     """Algorithmic bytes: number of distinct history cells (32 B each) that the type-1 and type-2
     lookups of one evaluation touch (computed from integer row / column indices only).  Exact over
     all targets when `sample` is None.  With a strided target sample the type-2 part is the per-row
@@ -74,28 +74,33 @@ def unique_cells(theta, omega, t, s, L, N, sample=None):
     that contains the first and the last target is that run up to the stride's resolution."""
     M = N - 1
     tM = t[M]
-    # type-1: rows n, n+1 of tau = theta_i t, all columns, all targets (cheap)
-    n1 = np.clip(np.searchsorted(t[:M], theta * tM, side="right") - 1, 0, M - 1)
+    # rows read around the interval [t_n, t_n+1): Hermite (window = 2): n, n+1; values-only history
+    # (window = 4, 4-point Lagrange in t): k .. k+3 with k = clamp(n-1, 0, M-3)
+    def first_row(n):
+        return n if window == 2 else np.clip(n - 1, 0, max(M - 3, 0))
+    nwin = 2 if window == 2 else min(4, M + 1)
+    # type-1: all columns, all targets (cheap)
+    n1 = first_row(np.clip(np.searchsorted(t[:M], theta * tM, side="right") - 1, 0, M - 1))
     full = np.zeros(N, dtype=bool)
-    full[n1] = True
-    full[n1 + 1] = True
+    for q in range(nwin):
+        full[n1 + q] = True
     idx = np.arange(L) if sample is None else sample
     touched = np.zeros((N, L), dtype=bool) if sample is None else None
     lo = np.full(N, L, dtype=np.int64)
     hi = np.full(N, -1, dtype=np.int64)
     for i in idx:
         phi2 = theta[i] + omega[i] * theta
-        n2 = np.clip(np.searchsorted(t[:M], phi2 * tM, side="right") - 1, 0, M - 1)
+        n2 = first_row(np.clip(np.searchsorted(t[:M], phi2 * tM, side="right") - 1, 0, M - 1))
         with np.errstate(invalid="ignore", divide="ignore"):
             psi = np.where(phi2 > 0, theta[i] / phi2, 0.0)
         lstar = np.searchsorted(theta, psi, side="right") - 1
         a3 = np.clip(lstar - (s // 2 - 1), 0, L - s)
         if touched is not None:
             for l in range(s):
-                touched[n2, a3 + l] = True
-                touched[n2 + 1, a3 + l] = True
+                for q in range(nwin):
+                    touched[n2 + q, a3 + l] = True
         else:
-            for rows in (n2, n2 + 1):
+            for rows in [n2 + q for q in range(nwin)]:
                 np.minimum.at(lo, rows, a3)
                 np.maximum.at(hi, rows, a3 + s - 1)
     if touched is not None:
@@ -158,7 +163,7 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------------------------------
 def oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, n_targets, seed=12345, min_seconds=0.0,
-                  max_reps=64):
+                  max_reps=64, values_only=False):
     """Time the CPU oracle (as it stands) on `n_targets` seeded targets x all L nodes; the same
     evaluation is repeated until `min_seconds` of CPU work have been timed.  Returns (targets per
     repetition, repetitions, seconds)."""
@@ -171,7 +176,8 @@ def oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, n_targets,
     reps, dt = 0, 0.0
     while reps < max_reps and (reps == 0 or dt < min_seconds):
         t0 = time.perf_counter()
-        O.history_integrals(grid, model, t, mu, hist, len(t) - 1, targets=targets, tables=tables)
+        (O.history_integrals_values if values_only else O.history_integrals)(
+            grid, model, t, mu, hist, len(t) - 1, targets=targets, tables=tables)
         dt += time.perf_counter() - t0
         reps += 1
     return len(targets), reps, dt
@@ -266,12 +272,15 @@ def run_ours(args):
     lo, hi, t_max, lam, T = WORKLOADS[args.workload]
     L, s = args.L, args.stencil
     N = L
-    ctx = D.dmfe_create(L, s, t_max, lam, T=T)
+    vo = bool(getattr(args, "values_only", False))
+    ctx = D.dmfe_create(L, s, t_max, lam, T=T, values_only=vo)
     tab = D.dmfe_get_tables(ctx, L, want_pairs=False)
     theta, omega, nu = tab["theta"], tab["omega"], tab["nu"]
     # every rank evaluates its own replica of the workload (weak scaling, no data-path collective:
     # DESIGN.md "Multi-GPU"); the seed is offset per rank so that the replicas are distinct problems
     t, mu, hist = inputs.synthetic_history(theta, omega, N, lo, hi, seed=replica_seed(rank))
+    if vo:   # the same fields without their slopes, 16-byte cells
+        hist = np.ascontiguousarray(hist[:, :, [0, 2]])
     tt, tm, th = (torch.from_numpy(a).to(dev) for a in (t, mu, hist))
     out = dict(d1C=torch.zeros(L, dtype=torch.float64, device=dev), d1R=torch.zeros(L, dtype=torch.float64, device=dev),
                mu_out=torch.zeros(1, dtype=torch.float64, device=dev),
@@ -364,12 +373,15 @@ def run_ours(args):
     # ---- roofline of the pair kernel ------------------------------------------------------------
     pairs = L * L
     fpp = flops_per_pair(s, lam)
+    if vo:   # 4-point Lagrange in t: no Hermite t-weights / slope terms, four rows instead of two
+        pmax_ = len(lam) - 1
+        fpp = (3 * (5 * s - 4) + 8 * s + 16 + 28 + 16 * s + 16 + 4 * 2 * max(pmax_ - 2, 0) + 3 * 2 * max(pmax_ - 1, 0) + 30)
     if L <= 8192:
-        cells, sampled = unique_cells(theta, omega, t, s, L, N), False
+        cells, sampled = unique_cells(theta, omega, t, s, L, N, window=4 if vo else 2), False
     else:
         samp = np.unique(np.append(np.arange(0, L, max(1, L // 1024)), L - 1))
-        cells, sampled = unique_cells(theta, omega, t, s, L, N, sample=samp), True
-    alg_bytes = 32 * cells + 8 * 8 * L
+        cells, sampled = unique_cells(theta, omega, t, s, L, N, sample=samp, window=4 if vo else 2), True
+    alg_bytes = (16 if vo else 32) * cells + 8 * 8 * L
     table_bytes = 24 * pairs
     peaks = {}
     try:
@@ -395,14 +407,15 @@ def run_ours(args):
     if traffic is None:
         try:   # dram bytes per launch of this kernel on this workload from the committed ncu capture
             import csv
-            key = "%s_L%d_s%d" % (args.workload, L, s)
+            key = "%s_L%d_s%d%s" % (args.workload, L, s, "_values" if vo else "")
             rows = {r["workload_key"]: r for r in csv.DictReader(open(os.path.join(ROOT, "profiles", "traffic.csv")))}
             traffic, traffic_src = float(rows[key]["dram_bytes_per_launch"]), rows[key]["source"]
         except Exception:
             traffic, traffic_src = None, None
     roof.update({
         "traffic": traffic, "traffic_source": traffic_src, "peak_source": "hbm: %s copy bandwidth; alu: DFMA chain measured in this run "
-        "on %d SMs" % (hbm_src, sms), "kernel": ("history_integrals_s4_kernel" if s == 4 else "history_integrals_kernel<%d>" % s),
+        "on %d SMs" % (hbm_src, sms), "kernel": ("history_integrals_values_kernel<%d>" % s if vo else
+                   ("history_integrals_s4_kernel" if s == 4 else "history_integrals_kernel<%d>" % s)),
         "kernel_ms_avg": k_avg_ms,
         "kernel_ms_min": k_min, "launches_timed": n_k, "algorithmic_bytes": alg_bytes,
         "algorithmic_bytes_sampled": sampled, "table_bytes": table_bytes, "flops_per_pair": fpp,
@@ -419,7 +432,8 @@ def run_ours(args):
 
     # ---- the oracle on this box's host cores, bounded sample -----------------------------------
     nt = args.ref_targets
-    n_s, reps, dt = oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, nt, min_seconds=args.ref_seconds)
+    n_s, reps, dt = oracle_sample(L, s, t_max, lam, T, theta, omega, nu, t, mu, hist, nt, min_seconds=args.ref_seconds,
+                                  values_only=vo)
     cpu = {"value": EVALS_PER_PAIR * n_s * L * reps / dt, "unit": UNIT, "cores": host_cores(), "kind": "oracle",
            "sample": "%d seeded targets x %d nodes of the same L=N=%d evaluation, repeated %d times (%.1f s of "
                      "CPU work)" % (n_s, L, L, reps, dt)}
@@ -447,8 +461,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "%s: single history-integral evaluation, L=N=%d log-spaced rows, s=%d, lambda=%s, T=%g"
-                   % (args.workload, L, s, lam, T), "pairs_per_step": pairs, "replicas": world,
+        "config": {"workload": "%s: single history-integral evaluation, L=N=%d log-spaced rows, s=%d, lambda=%s, T=%g%s"
+                   % (args.workload, L, s, lam, T, ", values-only history (4-point Lagrange in t)" if vo else ""), "pairs_per_step": pairs, "replicas": world,
                    "l2": ("inputs fit in L2 (%.0f MB history + %.0f MB pair tables): %d MB written to a scratch "
                           "buffer before every timed step, each step timed on its own"
                           % (hist.nbytes / 1e6, table_bytes / 1e6, FLUSH_BYTES >> 20)) if need_flush else
@@ -480,6 +494,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--traj-seconds", type=float, default=8.0,
                     help="wall-time budget of the adaptive trajectory segment (0 = skip)")
+    ap.add_argument("--values-only", action="store_true",
+                    help="values-only history with 4-point Lagrange in t (SURVEY.md 8(f)-2) instead of Hermite")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="dram bytes per launch of the pair kernel from the committed ncu capture (profiles/)")
     args = ap.parse_args()

@@ -58,6 +58,11 @@ typedef struct {
   double beta0;        /* inverse temperature of the initial condition, 0 = random start (Eq.(12)) */
   double tol;          /* epsilon of Eq.(25); used by rk_step / sparsify only      */
   double h_min;        /* terminate below this step; 0 -> 1e-12                    */
+  int32_t values_only; /* != 0: the history holds {C, R} only (16-byte cells, [n_cap][L][2]) and the
+                          interpolation in t is the local 4-point Lagrange polynomial through rows
+                          n-1 .. n+2 instead of cubic Hermite.
+                          dmfe_history_integrals(_host) only: the integrator calls return DMFE_EINVAL */
+  int32_t reserved;
   void *stream;        /* cudaStream_t borrowed from the caller (0 = default stream)             */
 } dmfe_params;
 
@@ -86,7 +91,7 @@ typedef struct {
   int32_t n_cap;      /* row capacity of the three arrays                                       */
   const double *t;    /* [n_cap] ascending, t[0] = 0                                            */
   const double *mu;   /* [n_cap] Lagrange multiplier of rows 0..M-1 (Eq.(13))                   */
-  const double *hist; /* [n_cap][L][4] packed cells {C, dC, R, dR}                              */
+  const double *hist; /* [n_cap][L][4] packed cells {C, dC, R, dR}; values_only: [n_cap][L][2] {C, R} */
 } dmfe_grid;
 
 /* Outputs of one right-hand-side evaluation; DEVICE pointers, any may be NULL. */

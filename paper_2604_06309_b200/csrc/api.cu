@@ -33,6 +33,7 @@ static void free_all(dmfe_ctx *c) {
   cudaFree(c->tab);
   cudaFree(c->blo);
   cudaFree(c->muw);
+  cudaFree(c->win);
   cudaFree(c->rowtab);
   cudaFree(c->br);
   cudaFree(c->jtop);
@@ -172,6 +173,7 @@ int dmfe_get_tables(dmfe_ctx *ctx, double *theta, double *omega, double *nu, int
 int dmfe_history_integrals(dmfe_ctx *ctx, const dmfe_grid *g, const dmfe_rhs_out *out) {
   if (!ctx || !g || !out) return DMFE_EINVAL;
   if (g->n_rows < 2 || g->n_rows > g->n_cap || !g->t || !g->mu || !g->hist) return DMFE_EINVAL;
+  if (ctx->p.values_only) return dmfe_launch_rhs_values(ctx, g->n_rows - 1, g->n_cap, g->t, g->mu, g->hist, out);
   return dmfe_launch_rhs(ctx, g->n_rows - 1, g->n_cap, g->t, g->mu, g->hist, out);
 }
 
@@ -179,6 +181,7 @@ int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const double *t, 
                                 const double *hist, double *d1C, double *d1R, double *mu, double *energy) {
   if (!ctx || n_rows < 2 || !t || !mu_hist || !hist) return DMFE_EINVAL;
   const int L = ctx->p.L;
+  const size_t cell = ctx->p.values_only ? 2 : 4;  // doubles per history cell
   if (n_rows > ctx->stage_rows) {
     cudaFree(ctx->stage_t);
     cudaFree(ctx->stage_mu);
@@ -188,14 +191,14 @@ int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const double *t, 
     ctx->stage_rows = 0;
     CUDA_TRY(ctx, cudaMalloc(&ctx->stage_t, sizeof(double) * (size_t)n_rows));
     CUDA_TRY(ctx, cudaMalloc(&ctx->stage_mu, sizeof(double) * (size_t)n_rows));
-    CUDA_TRY(ctx, cudaMalloc(&ctx->stage_hist, sizeof(double) * 4 * (size_t)L * (size_t)n_rows));
+    CUDA_TRY(ctx, cudaMalloc(&ctx->stage_hist, sizeof(double) * cell * (size_t)L * (size_t)n_rows));
     CUDA_TRY(ctx, cudaMalloc(&ctx->stage_out, sizeof(double) * (2 * (size_t)L + 2)));
     ctx->stage_rows = n_rows;
   }
   cudaStream_t s = ctx->stream;
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_t, t, sizeof(double) * (size_t)n_rows, cudaMemcpyHostToDevice, s));
   CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_mu, mu_hist, sizeof(double) * (size_t)n_rows, cudaMemcpyHostToDevice, s));
-  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_hist, hist, sizeof(double) * 4 * (size_t)L * (size_t)n_rows,
+  CUDA_TRY(ctx, cudaMemcpyAsync(ctx->stage_hist, hist, sizeof(double) * cell * (size_t)L * (size_t)n_rows,
                                 cudaMemcpyHostToDevice, s));
   dmfe_rhs_out o;
   memset(&o, 0, sizeof(o));
@@ -203,7 +206,9 @@ int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const double *t, 
   o.d1R = ctx->stage_out + L;
   o.mu = ctx->stage_out + 2 * L;
   o.energy = ctx->stage_out + 2 * L + 1;
-  const int rc = dmfe_launch_rhs(ctx, n_rows - 1, n_rows, ctx->stage_t, ctx->stage_mu, ctx->stage_hist, &o);
+  const int rc = ctx->p.values_only
+                     ? dmfe_launch_rhs_values(ctx, n_rows - 1, n_rows, ctx->stage_t, ctx->stage_mu, ctx->stage_hist, &o)
+                     : dmfe_launch_rhs(ctx, n_rows - 1, n_rows, ctx->stage_t, ctx->stage_mu, ctx->stage_hist, &o);
   if (rc != DMFE_OK) return rc;
   if (d1C) CUDA_TRY(ctx, cudaMemcpyAsync(d1C, o.d1C, sizeof(double) * (size_t)L, cudaMemcpyDeviceToHost, s));
   if (d1R) CUDA_TRY(ctx, cudaMemcpyAsync(d1R, o.d1R, sizeof(double) * (size_t)L, cudaMemcpyDeviceToHost, s));

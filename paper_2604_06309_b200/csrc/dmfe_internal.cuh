@@ -62,6 +62,8 @@ struct dmfe_ctx {
   // ---- O(L) scratch (device) ----
   double2 *cur;     // [L] {C, R} of the current row, packed for 16-byte gathers
   int32_t *blo;     // [L] per-call row bracket table: blo[c] = n(theta_c t_M)
+  double *win;      // values-only mode: [win_cap][8] per-call t-windows {t_k..t_k+3, inverse denominators}
+  int32_t win_cap;
   double2 *muw;     // [L] per call: mu(theta_c t_M) = muw.x + muw.y * mu(t_M)  (reading G11)
   double2 *rowtab;  // [rowtab_cap] per-call {t_n, 1 / (t_{n+1} - t_n)}
   // S = 4 only (pairs_s4.cuh), rebuilt per call by the pre-pass
@@ -160,6 +162,9 @@ struct dmfe_stage {
 
 // tables.cu
 int dmfe_build_tables(dmfe_ctx *ctx);
+// pairs_values.cu: the right-hand side on a values-only history (dmfe_params.values_only)
+int dmfe_launch_rhs_values(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, const double *mu_hist,
+                           const double *hist, const dmfe_rhs_out *out);
 // history_integrals.cu
 // stage: optional stage update run by the pre-pass; deriv_row: optional row of the history whose
 // derivative slots receive F (the derivative is stored with the appended row)

@@ -131,6 +131,7 @@ int dmfe_set_step_size(dmfe_ctx *ctx, dmfe_state *st, double h) {
 }
 
 int dmfe_dp_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *accepted) {
+  if (ctx && ctx->p.values_only) return DMFE_EINVAL;  // the integrator keeps the Hermite history
   if (!ctx || !st || !st->t || !st->mu || !st->hist) return DMFE_EINVAL;
   if (st->n_rows < 1) return DMFE_EINVAL;
   if (st->n_rows + 1 > st->n_cap) return DMFE_ECAPACITY;

@@ -116,6 +116,7 @@ int enqueue_step(dmfe_ctx *ctx, dmfe_state *st, int fixed_step, double *log, int
 extern "C" {
 
 int dmfe_init_state(dmfe_ctx *ctx, dmfe_state *st, double h0) {
+  if (ctx && ctx->p.values_only) return DMFE_EINVAL;  // the integrator keeps the Hermite history
   if (!ctx || !st || !st->t || !st->mu || !st->hist || st->n_cap < 3 || !(h0 > 0.0)) return DMFE_EINVAL;
   const int L = ctx->p.L;
   const double h = fmin(h0, ctx->h_stab);
@@ -133,6 +134,7 @@ int dmfe_init_state(dmfe_ctx *ctx, dmfe_state *st, double h0) {
 
 int dmfe_advance(dmfe_ctx *ctx, dmfe_state *st, int32_t n_steps, int32_t fixed_step, dmfe_advance_result *res,
                  double *step_log) {
+  if (ctx && ctx->p.values_only) return DMFE_EINVAL;  // the integrator keeps the Hermite history
   if (!ctx || !st || !st->t || !st->mu || !st->hist || n_steps < 1) return DMFE_EINVAL;
   if (st->n_rows < 1) return DMFE_EINVAL;
   if (st->n_rows + 1 > st->n_cap) return DMFE_ECAPACITY;

@@ -158,6 +158,7 @@ __global__ void sparsify_scatter_kernel(int L, int d0, int rows, const int32_t *
 
 extern "C" int dmfe_sparsify(dmfe_ctx *ctx, dmfe_state *st, int32_t protect_last, int32_t *n_rows_out,
                              uint8_t *keep_mask) {
+  if (ctx && ctx->p.values_only) return DMFE_EINVAL;  // the integrator keeps the Hermite history
   if (!ctx || !st || !st->t || !st->mu || !st->hist || protect_last < 0) return DMFE_EINVAL;
   const int L = ctx->p.L, N = st->n_rows;
   cudaStream_t s = ctx->stream;
