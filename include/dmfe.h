@@ -119,7 +119,9 @@ DMFE_API int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const do
                                 const double *hist, double *d1C, double *d1R, double *mu,
                                 double *energy);
 
-/* Device-resident integrator state.  The arrays are caller-owned DEVICE memory. */
+/* Device-resident integrator state.  The arrays are caller-owned DEVICE memory.  The device copies of the
+ * step size, the row count and the decisions live in the context: a context drives ONE state at a time
+ * (dmfe_init_state or any call with another state's arrays re-synchronises from the host fields below). */
 typedef struct {
   int32_t n_rows;  /* complete rows (value + derivative + mu); updated by the library            */
   int32_t n_cap;   /* capacity; a step needs n_rows + 1 <= n_cap                                  */

@@ -158,7 +158,7 @@ void orc_mu_energy(int L, int M, const double *lam, int pmax, double T, double b
  *  rows2    [nt][L]  type-2 row index n(phi2_ij t)
  *  mu_out, E_out     Eq.(13), Eq.(14)
  */
-void orc_history_integrals(int L, int s, int M, const double *lam, int pmax, double T,
+static void history_integrals_worker(int logR, int L, int s, int M, const double *lam, int pmax, double T,
                            double beta0, const double *theta, const double *omega,
                            const double *nu, const double *t, const double *mu_hist,
                            const double *hist, int nt, const int32_t *targets,
@@ -208,8 +208,16 @@ void orc_history_integrals(int L, int s, int M, const double *lam, int pmax, dou
             /* ---- type-1 lookup: B(theta_i t, theta_j), t-interpolation only (Eq.19) ---- */
             const double B1C = h1[0] * HC(n1, j) + h1[1] * HDC(n1, j) +
                                h1[2] * HC(n1 + 1, j) + h1[3] * (n1 + 1 == M ? 0.0 : HDC(n1 + 1, j));
-            const double B1R = h1[0] * HR(n1, j) + h1[1] * HDR(n1, j) +
-                               h1[2] * HR(n1 + 1, j) + h1[3] * (n1 + 1 == M ? 0.0 : HDR(n1 + 1, j));
+            double B1R = h1[0] * HR(n1, j) + h1[1] * HDR(n1, j) +
+                         h1[2] * HR(n1 + 1, j) + h1[3] * (n1 + 1 == M ? 0.0 : HDR(n1 + 1, j));
+            if (logR && HR(n1, j) > 0.0 && HR(n1 + 1, j) > 0.0) {
+                /* logarithmic interpolation of the response history: the same
+                 * interpolant applied to log R with the scaled slope dR/R; reading G32 */
+                const double ell = h1[0] * log(HR(n1, j)) + h1[1] * (HDR(n1, j) / HR(n1, j)) +
+                                   h1[2] * log(HR(n1 + 1, j)) +
+                                   h1[3] * (n1 + 1 == M ? 0.0 : HDR(n1 + 1, j) / HR(n1 + 1, j));
+                B1R = exp(ell);
+            }
             if (j == 0) B1C_first = B1C;
             /* ---- type-2 lookup: B(phi2 t, theta_i/phi2): theta-stencil first, then t (Eq.20) ---- */
             const double phi2 = th_i + om_i * theta[j];
@@ -232,7 +240,24 @@ void orc_history_integrals(int L, int s, int M, const double *lam, int pmax, dou
                 }
             }
             const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
-            const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
+            double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
+            if (logR) {
+                /* all 2 s stencil values positive: theta-stencil and t-interpolant on log R and dR/R;
+                 * otherwise the ordinary interpolation above stands ("automatic fallback") */
+                int positive = 1;
+                for (int l = 0; l < s; ++l)
+                    if (!(HR(n2, a3 + l) > 0.0) || !(HR(n2 + 1, a3 + l) > 0.0)) positive = 0;
+                if (positive) {
+                    double ll = 0.0, dll = 0.0, lu = 0.0, dlu = 0.0;
+                    for (int l = 0; l < s; ++l) {
+                        ll += w3[l] * log(HR(n2, a3 + l));
+                        dll += w3[l] * (HDR(n2, a3 + l) / HR(n2, a3 + l));
+                        lu += w3[l] * log(HR(n2 + 1, a3 + l));
+                        if (n2 + 1 != M) dlu += w3[l] * (HDR(n2 + 1, a3 + l) / HR(n2 + 1, a3 + l));
+                    }
+                    B2R = exp(h2[0] * ll + h2[1] * dll + h2[2] * lu + h2[3] * dlu);
+                }
+            }
             /* ---- kernel functions (Eq.10, Eq.11) and the eight terms (Eq.21) ---- */
             const double nj = nu[j];
             double term[8];
@@ -281,6 +306,32 @@ void orc_history_integrals(int L, int s, int M, const double *lam, int pmax, dou
         }
     }
     free(mu_all);
+}
+
+void orc_history_integrals(int L, int s, int M, const double *lam, int pmax, double T,
+                           double beta0, const double *theta, const double *omega,
+                           const double *nu, const double *t, const double *mu_hist,
+                           const double *hist, int nt, const int32_t *targets,
+                           const int32_t *start, const double *frac, double *sums,
+                           double *abssums, double *deriv, double *scale, int32_t *rows1,
+                           int32_t *rows2, double *mu_out, double *E_out) {
+    history_integrals_worker(0, L, s, M, lam, pmax, T, beta0, theta, omega, nu, t, mu_hist, hist, nt,
+                             targets, start, frac, sums, abssums, deriv, scale, rows1, rows2, mu_out, E_out);
+}
+
+/* The same with logarithmic interpolation of the response history (reading G32 in
+ * DESIGN.md): in the type-1 and type-2 lookups the interpolant acts on log R and on the scaled slope
+ * dR/R and the result is exponentiated, whenever every R value it reads is positive; otherwise the
+ * ordinary interpolation is used.  The A factors (current slice) are interpolated as before. */
+void orc_history_integrals_logr(int L, int s, int M, const double *lam, int pmax, double T,
+                           double beta0, const double *theta, const double *omega,
+                           const double *nu, const double *t, const double *mu_hist,
+                           const double *hist, int nt, const int32_t *targets,
+                           const int32_t *start, const double *frac, double *sums,
+                           double *abssums, double *deriv, double *scale, int32_t *rows1,
+                           int32_t *rows2, double *mu_out, double *E_out) {
+    history_integrals_worker(1, L, s, M, lam, pmax, T, beta0, theta, omega, nu, t, mu_hist, hist, nt,
+                             targets, start, frac, sums, abssums, deriv, scale, rows1, rows2, mu_out, E_out);
 }
 
 /* Sparsification residual (Eq.(26)-(27)): for every interior row n

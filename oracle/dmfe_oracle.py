@@ -193,7 +193,7 @@ class Grid:
 
 # --------------------------------------------------------------------------- history integrals
 def history_integrals(grid: Grid, model: Model, t, mu_hist, hist, M: int, targets=None,
-                      tables=None, want_rows=False):
+                      tables=None, want_rows=False, log_r=False):
     """The per-stage right-hand side: Eq.(17)-(21), Eq.(13), Eq.(14), Eq.(1).
 
     t[0..M], mu_hist[0..M-1], hist[(M+1), L, 4] = {C, dC, R, dR}; row M values only.
@@ -220,7 +220,8 @@ def history_integrals(grid: Grid, model: Model, t, mu_hist, hist, M: int, target
     rows1 = np.zeros(nt, dtype=np.int32) if want_rows else None
     rows2 = np.zeros((nt, L), dtype=np.int32) if want_rows else None
     mu = ctypes.c_double(0.0); E = ctypes.c_double(0.0)
-    lib.orc_history_integrals(
+    # log_r: logarithmic interpolation of the response history (reading G32)
+    (lib.orc_history_integrals_logr if log_r else lib.orc_history_integrals)(
         ctypes.c_int(L), ctypes.c_int(s), ctypes.c_int(M), _p(model.lam), ctypes.c_int(model.pmax),
         ctypes.c_double(model.T), ctypes.c_double(model.beta0), _p(grid.theta), _p(grid.omega),
         _p(grid.nu), _p(t), _p(mu_hist), _p(hist), ctypes.c_int(nt), _p(targets), _p(start),

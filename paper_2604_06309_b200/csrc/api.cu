@@ -73,6 +73,7 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
   if (!c) return DMFE_ENOMEM;
   memset(c, 0, sizeof(*c));
   c->p = p;
+  c->rowtab_dirty = 1;
   if (c->p.h_min <= 0.0) c->p.h_min = 1e-12;
   c->stream = (cudaStream_t)p.stream;
   ModelCoef &m = c->model;

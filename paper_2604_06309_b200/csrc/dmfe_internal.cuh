@@ -43,6 +43,7 @@ enum {
   IS_NACC = 4,    // accepted / reverted / attempted steps of the running dmfe_advance call
   IS_NREV = 5,
   IS_STEP = 6,
+  IS_RTVALID = 7, // leading entries of the per-call row table that are final (device-resident steps)
   IS_COUNT = 8
 };
 
@@ -72,6 +73,7 @@ struct dmfe_ctx {
   double *coefM;    // [L][8]  centred cubics of {C, R} of the current row, per stencil start
   double *coefT;    // [L][16] centred cubics of {C, dC, R, dR} of row M-1
   int32_t rowtab_cap;
+  int rowtab_dirty;  // the row table was (or may have been) rebuilt for another history: rebuild it in full
   double *scal;     // [SC_COUNT]
   int32_t *iscal;   // [IS_COUNT]
   double *rk;       // [4][L][2]: q1, q2, delta, F

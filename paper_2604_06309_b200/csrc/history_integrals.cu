@@ -90,7 +90,12 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
     const int nb = gridDim.x == 1 ? 1 : gridDim.x - 1;
     const int b = gridDim.x == 1 ? 0 : blockIdx.x - 1;
     const int n_extra = s4.on ? 2 * L - 3 : 0;  // jtop [L] and coefT [L-3]
-    for (int e = b * PREP_THREADS + threadIdx.x; e < M + L + n_extra; e += nb * PREP_THREADS) {
+    // rows below rt0 already have their final row-table entries (device-resident steps: only the
+    // entries at the end of the history change between evaluations; rk_step.cu keeps the count)
+    const int rt0 = sg.dev_rows ? min(max(sg.iscal[IS_RTVALID], 0), M - 1) : 0;
+    const int n_rt = M - rt0;
+    for (int e0 = b * PREP_THREADS + threadIdx.x; e0 < n_rt + L + n_extra; e0 += nb * PREP_THREADS) {
+      const int e = e0 + rt0;  // item index as if every row-table entry were rebuilt
       if (e < M) {
         const double tn = t[e];
         const double tn1 = (e + 1 == M) ? tM : t[e + 1];
@@ -292,6 +297,7 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
     CUDA_TRY(ctx, cudaMalloc(&ctx->rowtab, sizeof(double2) * (size_t)cap));
     ctx->rowtab_cap = cap;
   }
+  if (!(stage && stage->dev_rows)) ctx->rowtab_dirty = 1;  // host-driven evaluation: full rebuild, here and next time
   const bool s4 = ctx->p.stencil == 4;
   int pb = 1 + (M + (s4 ? 3 : 1) * L + PREP_THREADS - 1) / PREP_THREADS;
   if (pb > 33) pb = 33;

@@ -21,13 +21,6 @@
 namespace dmfe_rhs {
 
 
-// Small per-call tables (current row, row table, bracket table) live in shared memory when they
-// fit (SM = true): the gathers into them are the head of every pair's dependent load chain.
-template <bool SM, class T>
-__device__ __forceinline__ T ld_tab(const T *p) {
-  return *p;
-}
-
 // n = max{ n in [lo, hi] : rowtab[n].x <= tau }; requires t[lo] <= tau.
 __device__ __forceinline__ int row_search_tab(const double2 *rowtab, int lo, int hi, double tau) {
   while (lo < hi) {

@@ -61,6 +61,13 @@ __global__ void commit_step_kernel(int32_t *__restrict__ iscal, double *__restri
     n = (n - 10 > 1) ? n - 10 : 1;  // revert the previous ten steps
     iscal[IS_NREV] += 1;
   }
+  // row-table entries below the last complete row of the step that has just run are final; after a
+  // revert only those below the new last row
+  {
+    const int n_before = acc ? n - 1 : iscal[IS_NROWS];
+    const int v = (n < n_before ? n : n_before) - 1;
+    iscal[IS_RTVALID] = v > 0 ? v : 0;
+  }
   iscal[IS_NROWS] = n;
   scal[SC_TLAST] = t[n - 1];
   const int step = iscal[IS_STEP];
@@ -73,7 +80,8 @@ __global__ void commit_step_kernel(int32_t *__restrict__ iscal, double *__restri
   iscal[IS_STATUS] = status;
 }
 
-__global__ void begin_batch_kernel(int32_t *__restrict__ iscal, int n_rows) {
+__global__ void begin_batch_kernel(int32_t *__restrict__ iscal, int n_rows, int rowtab_dirty) {
+  if (rowtab_dirty) iscal[IS_RTVALID] = 0;
   iscal[IS_NROWS] = n_rows;
   iscal[IS_STATUS] = 0;
   iscal[IS_NACC] = 0;
@@ -123,6 +131,7 @@ int dmfe_init_state(dmfe_ctx *ctx, dmfe_state *st, double h0) {
   init_row0_kernel<<<(L + 255) / 256, 256, 0, ctx->stream>>>(L, ctx->model, ctx->omega, st->hist, st->t, st->mu,
                                                            st->energy, ctx->scal, h);
   CUDA_TRY(ctx, cudaGetLastError());
+  ctx->rowtab_dirty = 1;
   st->n_rows = 1;
   st->h = h;
   st->eps_rk = 0.0;
@@ -165,7 +174,8 @@ int dmfe_advance(dmfe_ctx *ctx, dmfe_state *st, int32_t n_steps, int32_t fixed_s
     CUDA_TRY(ctx, cudaMalloc(&ctx->rowtab, sizeof(double2) * (size_t)st->n_cap));
     ctx->rowtab_cap = st->n_cap;
   }
-  begin_batch_kernel<<<1, 1, 0, s>>>(ctx->iscal, st->n_rows);
+  begin_batch_kernel<<<1, 1, 0, s>>>(ctx->iscal, st->n_rows, ctx->rowtab_dirty);
+  ctx->rowtab_dirty = 0;
   CUDA_TRY(ctx, cudaGetLastError());
   // one step as a graph, captured once per (state arrays, mode); plain launches if capture is unavailable
   const void *key[5] = {st->t, st->mu, st->energy, st->hist,

@@ -229,6 +229,7 @@ extern "C" int dmfe_sparsify(dmfe_ctx *ctx, dmfe_state *st, int32_t protect_last
   }
   CUDA_TRY(ctx, cudaStreamSynchronize(s));
   st->n_rows = ctx->h_iscal[IS_NROWS];
+  ctx->rowtab_dirty = 1;  // the rows moved
   if (n_rows_out) *n_rows_out = st->n_rows;
   return DMFE_OK;
 }

@@ -20,6 +20,9 @@ CONFIGS = {
     # BASELINE.json configs[2], [3] (sizes: DESIGN.md section 4)
     3: dict(lam=[0.0, 0.0, 1.0, 0.0, 0.5], T=0.5, tol=1e-8, n_cap=2048, t_max=1e5, L=512, s=4),
     4: dict(lam=[0.0, 0.0, 0.0, 1.0], T=0.5, tol=1e-8, n_cap=8192, t_max=1e7, L=512, s=4),
+    # SURVEY.md 8(f)-4, second workload: the 3+9 model at lambda = 1/2 quenched to T = 0 (Fig. 3,
+    # :410 Fig. 8), f = (q^3 + q^9)/4 in the convention f = 1/2 sum lam_p q^p; run-time degree of f (p_max > 4)
+    39: dict(lam=[0.0, 0.0, 0.0, 0.5, 0.0, 0.0, 0.0, 0.0, 0.0, 0.5], T=0.0, tol=1e-8, n_cap=32768, t_max=1e5, L=512, s=4),
 }
 
 
@@ -119,6 +122,9 @@ def run(L, s, t_max, lam, T, tol, n_cap, t_end, h0=1e-3, sp_every=200, protect_l
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
+    ap.add_argument("--beta0", type=float, default=0.0, help="inverse temperature of the initial condition (Eq.(12))")
+    ap.add_argument("--tol", type=float, default=None)
+    ap.add_argument("--stencil", type=int, default=None)
     ap.add_argument("--t-end", type=float, default=1e3)
     ap.add_argument("--L", type=int, default=None)
     ap.add_argument("--n-cap", type=int, default=None, help="row capacity (default: the config's hard cap)")
@@ -132,6 +138,11 @@ def main():
         cfg["L"] = args.L
     if args.n_cap:
         cfg["n_cap"] = args.n_cap
+    if args.tol:
+        cfg["tol"] = args.tol
+    if args.stencil:
+        cfg["s"] = args.stencil
+    cfg["beta0"] = args.beta0
     progress = None
     if args.log:
         def progress(rec, stats):
