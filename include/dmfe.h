@@ -62,7 +62,10 @@ typedef struct {
                           interpolation in t is the local 4-point Lagrange polynomial through rows
                           n-1 .. n+2 instead of cubic Hermite.
                           dmfe_history_integrals(_host) only: the integrator calls return DMFE_EINVAL */
-  int32_t reserved;
+  int32_t log_r;       /* != 0: logarithmic interpolation of the response history: the type-1
+                          and type-2 lookups of R act on log R and dR/R whenever every value read is
+                          positive, with automatic fallback to the ordinary interpolation (reading G32);
+                          not with values_only                                                        */
   void *stream;        /* cudaStream_t borrowed from the caller (0 = default stream)             */
 } dmfe_params;
 

@@ -69,6 +69,7 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
   if (!(p.t_max > 2.718281828459045)) return DMFE_EINVAL;
   if (p.p_max < 2 || p.p_max > DMFE_PMAX_MAX) return DMFE_EINVAL;
   if (!(T >= 0.0) || !(p.beta0 >= 0.0) || !(p.tol >= 0.0)) return DMFE_EINVAL;
+  if (p.values_only && p.log_r) return DMFE_EINVAL;
   dmfe_ctx *c = new (std::nothrow) dmfe_ctx;
   if (!c) return DMFE_ENOMEM;
   memset(c, 0, sizeof(*c));

@@ -298,7 +298,7 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
     ctx->rowtab_cap = cap;
   }
   if (!(stage && stage->dev_rows)) ctx->rowtab_dirty = 1;  // host-driven evaluation: full rebuild, here and next time
-  const bool s4 = ctx->p.stencil == 4;
+  const bool s4 = ctx->p.stencil == 4 && !ctx->p.log_r;  // the log-R option runs the generic kernel
   int pb = 1 + (M + (s4 ? 3 : 1) * L + PREP_THREADS - 1) / PREP_THREADS;
   if (pb > 33) pb = 33;
   dmfe_stage sg;

@@ -38,6 +38,27 @@ int dmfe_launch_pairs_generic(dmfe_ctx *ctx, const RhsArgs &a, int grid) {
     else                     \
       DMFE_LAUNCH_G(S_, 0);  \
   } while (0)
+#define DMFE_LAUNCH_LOG(S_)                                          \
+  do {                                                              \
+    if (mode == 2)                                                  \
+      DMFE_LAUNCH_K((history_integrals_kernel<S_, 0, 2, true>));    \
+    else if (mode == 1)                                             \
+      DMFE_LAUNCH_K((history_integrals_kernel<S_, 0, 1, true>));    \
+    else                                                            \
+      DMFE_LAUNCH_K((history_integrals_kernel<S_, 0, 0, true>));    \
+  } while (0)
+  if (ctx->p.log_r) {  // logarithmic interpolation of the response history: run-time degree of f only
+    switch (ctx->p.stencil) {
+      case 2: DMFE_LAUNCH_LOG(2); break;
+      case 4: DMFE_LAUNCH_LOG(4); break;
+      case 6: DMFE_LAUNCH_LOG(6); break;
+      case 8: DMFE_LAUNCH_LOG(8); break;
+      case 10: DMFE_LAUNCH_LOG(10); break;
+      default: return DMFE_EINVAL;
+    }
+    return DMFE_OK;
+  }
+#undef DMFE_LAUNCH_LOG
   switch (ctx->p.stencil) {
     case 2: DMFE_LAUNCH_GS(2); break;
     case 6: DMFE_LAUNCH_GS(6); break;

@@ -51,7 +51,10 @@ __device__ __forceinline__ int index_stage(const double2 *rowtab, const int32_t 
 }
 
 // SM: 0 = per-call tables read from global memory, 1 = cur and blo in shared memory, 2 = rowtab too
-template <int S, int PD, int SM>
+// LOGR: logarithmic interpolation of the response history (reading G32): in the type-1 and
+// type-2 lookups the interpolant acts on log R and dR/R whenever every R value it reads is positive and the
+// result is exponentiated; otherwise the ordinary interpolation stands.
+template <int S, int PD, int SM, bool LOGR = false>
 __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsArgs a, ModelCoef mc) {
   constexpr bool SMT = SM >= 1, SMR = SM == 2;
   extern __shared__ double4 smem_dyn[];
@@ -144,7 +147,9 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         }
         if (top1) hi.y = 0.0, hi.w = 0.0;
         const double B1C = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
-        const double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
+        double B1R = h1[0] * lo.z + h1[1] * lo.w + h1[2] * hi.z + h1[3] * hi.w;
+        if (LOGR && lo.z > 0.0 && hi.z > 0.0)
+          B1R = exp(h1[0] * log(lo.z) + h1[1] * (lo.w / lo.z) + h1[2] * log(hi.z) + h1[3] * (hi.w / hi.z));
         if (j == 0) b1c_first = B1C;
         // every term carries nu_j and exactly one of R1, B1R: fold nu_j into those two
         const double nR1 = nuA * R1, nB1R = nuA * B1R;
@@ -221,9 +226,18 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         // theta-stencil first, then t
         lagrange_weights<S>(u3, w);
         double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
+        double ll = 0.0, dll = 0.0, lu = 0.0, dlu = 0.0;
+        bool positive = true;
 #pragma unroll
         for (int l = 0; l < S; ++l) {
           const double4 xl = x[l], yl = ld_cell(p2 + L + l);
+          if (LOGR) {
+            positive = positive && (xl.z > 0.0) && (yl.z > 0.0);
+            ll = fma(w[l], log(xl.z), ll);
+            dll = fma(w[l], xl.w / xl.z, dll);
+            lu = fma(w[l], log(yl.z), lu);
+            dlu = fma(w[l], yl.w / yl.z, dlu);
+          }
           cl = fma(w[l], xl.x, cl);
           dcl = fma(w[l], xl.y, dcl);
           rl = fma(w[l], xl.z, rl);
@@ -235,7 +249,11 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
         }
         if (top2) dcu = 0.0, dru = 0.0;
         const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
-        const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
+        double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
+        if (LOGR && positive) {
+          if (top2) dlu = 0.0;
+          B2R = exp(h2[0] * ll + h2[1] * dll + h2[2] * lu + h2[3] * dlu);
+        }
         const double nR2 = nj * R2;
         const double K2 = f2<PD>(mc, C2) * nR2;
         acc[0] = fma(K2, B2C, acc[0]);                     // S2: K(t,s) C(s,t')

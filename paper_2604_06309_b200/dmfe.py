@@ -27,7 +27,7 @@ EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror
 class dmfe_params(Structure):
     _fields_ = [("L", c_int32), ("stencil", c_int32), ("quad_degree", c_int32), ("p_max", c_int32),
                 ("t_max", c_double), ("beta0", c_double), ("tol", c_double), ("h_min", c_double),
-                ("values_only", c_int32), ("reserved", c_int32), ("stream", c_void_p)]
+                ("values_only", c_int32), ("log_r", c_int32), ("stream", c_void_p)]
 
 
 class dmfe_grid(Structure):
@@ -152,7 +152,7 @@ def _host(a):
 
 # ------------------------------------------------------------------------------------------------
 def dmfe_create(L, stencil, t_max, lam, T, beta0=0.0, tol=0.0, h_min=0.0, quad_degree=5, stream=None,
-                values_only=False):
+                values_only=False, log_r=False):
     """-> opaque context handle.  lam[p] are the lambda_p of f(q) = 1/2 sum_p lam[p] q^p."""
     import torch
     lib = load_library()
@@ -162,7 +162,7 @@ def dmfe_create(L, stencil, t_max, lam, T, beta0=0.0, tol=0.0, h_min=0.0, quad_d
     if stream is None:
         stream = torch.cuda.current_stream().cuda_stream
     p = dmfe_params(L=L, stencil=stencil, quad_degree=quad_degree, p_max=len(lam) - 1, t_max=t_max, beta0=beta0,
-                    tol=tol, h_min=h_min, values_only=1 if values_only else 0, reserved=0, stream=c_void_p(stream))
+                    tol=tol, h_min=h_min, values_only=1 if values_only else 0, log_r=1 if log_r else 0, stream=c_void_p(stream))
     ctx = c_void_p()
     _check(lib.dmfe_create(byref(p), lam.ctypes.data_as(POINTER(c_double)), float(T), byref(ctx)), "dmfe_create")
     return ctx

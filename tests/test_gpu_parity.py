@@ -266,6 +266,38 @@ def test_rhs_closed_form_constant_history_full_size_all_targets(D):
     assert np.abs(g["F"][:, 0] - FC).max() < tol and np.abs(g["F"][:, 1] - FR).max() < tol
 
 
+@pytest.mark.parametrize("L,N,s,lam,T,t_max,t_end,poison", [
+    (96, 37, 4, [0, 0, 0, 1.0], 1.0, 50.0, 30.0, False),
+    (100, 23, 6, [0, 0, 1.0, 0, 0.5], 0.5, 1e3, 200.0, True),
+    (130, 41, 10, [0, 0, 1.0, 0.8, 0.5], 0.7, 1e2, 60.0, True),
+    (64, 3, 2, [0, 0, 0, 1.0], 1.0, 10.0, 0.02, False),
+])
+def test_rhs_log_response_interpolation(D, L, N, s, lam, T, t_max, t_end, poison):
+    """dmfe_params.log_r (reading G32): logarithmic interpolation of the response history with
+    automatic fallback, against the oracle's orc_history_integrals_logr; `poison` plants non-positive response
+    values so that both branches run inside one evaluation."""
+    ctx = D.dmfe_create(L, s, t_max, lam, T=T, log_r=True)
+    try:
+        tab = D.dmfe_get_tables(ctx, L)
+        grid = _oracle_grid_from_library(tab, L, s, t_max)
+        t, mu, hist = inputs.random_smooth_history(tab["theta"], tab["omega"], N, t_end, seed=L + N)
+        if poison:
+            rng = np.random.Generator(np.random.PCG64(N))
+            for _ in range(40):
+                hist[rng.integers(0, N - 1), rng.integers(0, L), 2] *= -1.0
+            hist[N // 2, L // 3, 2] = 0.0
+        g = gpu_rhs(D, ctx, L, t, mu, hist, N)
+    finally:
+        D.dmfe_destroy(ctx)
+    model = O.Model(np.array(lam, dtype=np.float64), T, 0.0)
+    ref = O.history_integrals(grid, model, t, mu, hist, N - 1, tables=(tab["start"], tab["frac"]), want_rows=True,
+                              log_r=True)
+    ref["theta"] = tab["theta"]
+    compare_rhs(g, ref)
+    plain = O.history_integrals(grid, model, t, mu, hist, N - 1, tables=(tab["start"], tab["frac"]))
+    assert np.abs(plain["sums"] - ref["sums"]).max() > 1e-9 * np.abs(ref["abssums"]).max()   # the option is live
+
+
 def test_rhs_rows_in_a_larger_buffer(D):
     """n_rows < n_cap: rows beyond the current one are never touched (filled with NaN here)."""
     L, N, s = 80, 20, 4
