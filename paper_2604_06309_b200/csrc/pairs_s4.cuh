@@ -15,8 +15,8 @@
 //     cubics of its last stencil start in registers: psi = theta_i / phi2 moves by less than a grid
 //     cell over the top interval for most targets, so most top pairs load nothing but their table
 //     entries.
-//  2. The general loop (j < jtop[i], n2 <= M-2: both rows complete) finds n2 by probing upward from
-//     the lower end of the bracket br[a2] (n2 - lo is 0 for 85 % of the pairs, <= 2 for 99.9 %),
+//  2. The general loop (j < jtop[i], n2 <= M-2: both rows complete) finds n2 inside the bracket br[a2]
+//     (bisection while it is wide, then probing upward: n2 - lo is 0 for 85 % of the pairs when M ~ L),
 //     one pair ahead, while the lower-row cells of the current pair are in flight.
 //  3. Pair-table entries are requested two pairs ahead, type-1 cells one pair ahead.
 #pragma once
@@ -61,6 +61,21 @@ __device__ __forceinline__ double2 a_factor(const double2 *cur, uint64_t e) {
   const double2 y0 = cur[a], y1 = cur[a + 1], y2 = cur[a + 2], y3 = cur[a + 3];
   return make_double2(fma(w[3], y3.x, fma(w[2], y2.x, fma(w[1], y1.x, w[0] * y0.x))),
                       fma(w[3], y3.y, fma(w[2], y2.y, fma(w[1], y1.y, w[0] * y0.y))));
+}
+
+// n = max{ n in [lo, hi] : rowtab[n].x <= tau } (requires t[lo] <= tau): bisection while the
+// bracket is wide (histories with many more rows than grid nodes: a grid cell of phi2 spans ~ M/L rows),
+// then probing upward (M ~ L: the bracket holds 1 - 3 rows and n - lo is 0 for 85 % of the pairs)
+__device__ __forceinline__ int probe_row(const double2 *rowtab, int lo, int hi, double tau) {
+  while (hi - lo > 2) {
+    const int mid = lo + ((hi - lo + 1) >> 1);
+    if (rowtab[mid].x <= tau)
+      lo = mid;
+    else
+      hi = mid - 1;
+  }
+  while (lo < hi && rowtab[lo + 1].x <= tau) ++lo;
+  return lo;
 }
 
 template <int PD, int SM, bool HOOKS>
@@ -232,8 +247,7 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
         {
           tau2_c = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn_c.x)), tM);
           const int2 b = br[tab_start(e2_c)];
-          int n = b.x;
-          while (n < b.y && rowtab[n + 1].x <= tau2_c) ++n;
+          const int n = probe_row(rowtab, b.x, b.y, tau2_c);
           n2_c = n;
           rt_c = rowtab[n];
         }
@@ -251,8 +265,7 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
           if (k + 1 < Kg) {
             tau2_n = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn_n.x)), tM);
             const int2 b = br[tab_start(e2_n)];
-            int n = b.x;
-            while (n < b.y && rowtab[n + 1].x <= tau2_n) ++n;
+            const int n = probe_row(rowtab, b.x, b.y, tau2_n);
             n2_n = n;
             rt_n = rowtab[n];
           }
