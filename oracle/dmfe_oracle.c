@@ -7,7 +7,7 @@
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference legs may load it.
  *
- * What it follows, in the paper's order and notation (readings G1..G29 are
+ * What it follows, in the paper's order and notation (readings G1..G32 are
  * listed in DESIGN.md):
  *   Eq.(17)  PAPER.md:238-245  integrals I1 on [0,theta], I2 on [theta,1] with
  *            nodes phi1_ij = theta_i*theta_j, phi2_ij = theta_i + (1-theta_i)*theta_j
@@ -19,6 +19,10 @@
  *   Eq.(14)  PAPER.md:147      E(t)
  *   Eq.(1)   PAPER.md:69-75    dC/dt, dR/dt (with the -mu terms of Eq.(6), reading G1)
  *   Eq.(26)-(27) PAPER.md:326-332 sparsification residual
+ *   PAPER.md:435      values-only history, 4-point Lagrange in t (orc_history_integrals_values,
+ *                     reading G30; pins V1-V4)
+ *   PAPER.md:453      logarithmic interpolation of the response history with fallback
+ *                     (orc_history_integrals_logr, reading G32; pins LR1-LR4)
  *
  * Floating point: every product/sum below is a separate IEEE fp64 operation
  * (compile with -ffp-contract=off); the eight sums over j accumulate in

@@ -12,8 +12,10 @@ P8 uniform-grid brute force, P9 RK order conditions, P10 the numbers printed in 
 (tests/test_oracle_golden.py), P11-P14 Dormand-Prince start-up (tests/test_oracle_dp.py), P15 the beta0 forcing
 path (equilibrium start beta0 = 1/T is stationary from the first step: mu, E, time-translation invariance, FDT),
 orc_mu_at (cubic reproduction, window placement), the controller constants of PAPER.md:320 on a stubbed error
-sequence.  "parity unpinned": controller tie-breaks and the sparsification schedule (paper silent; readings G20,
-G25 in DESIGN.md).
+sequence, the greedy thinning walk (brute force over flag patterns) and the step loop `integrate` (tests/test_oracle_traj.py),
+V1-V4 the values-only history (tests/test_oracle_values.py), LR1-LR4 the log-R option (tests/test_oracle_logr.py).
+"parity unpinned": controller tie-breaks and the sparsification schedule (paper silent; readings G20,
+G25, G31 in DESIGN.md).
 """
 from __future__ import annotations
 
