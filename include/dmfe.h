@@ -42,6 +42,7 @@ extern "C" {
 #define DMFE_ESTEPMIN (-4)    /* controller drove h below h_min                    */
 #define DMFE_ENONFINITE (-5)  /* eps_RK not finite and nothing left to revert                     */
 #define DMFE_ENOMEM (-6)      /* host or device allocation failed                                 */
+#define DMFE_ETOOLARGE (-7)   /* dmfe_history_integrals_static: L or n_rows beyond the static scratch */
 
 typedef struct dmfe_ctx dmfe_ctx; /* opaque: tables + O(L) scratch on the device */
 
@@ -121,6 +122,29 @@ DMFE_API int dmfe_history_integrals(dmfe_ctx *ctx, const dmfe_grid *grid, const 
 DMFE_API int dmfe_history_integrals_host(dmfe_ctx *ctx, int32_t n_rows, const double *t, const double *mu_hist,
                                 const double *hist, double *d1C, double *d1R, double *mu,
                                 double *energy);
+
+/* The north-star call for callers that may not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same kernels and same results as dmfe_history_integrals
+ * (Eq.(17)-(21); Hermite history, any stencil, log_r honoured; values_only: DMFE_EINVAL), but the per-call
+ * tables of the pre-pass live in one file-scope device array of fixed size instead of context memory that
+ * the ordinary path grows with cudaMalloc on demand.  Limits: L <= DMFE_STATIC_MAX_L grid nodes and
+ * n_rows - 1 <= DMFE_STATIC_MAX_ROWS history rows, beyond which the call returns DMFE_ETOOLARGE and
+ * launches nothing; the array is 1 245 440 bytes and every GPU that loads the library holds it until the
+ * process exits.  The call issues two cudaMemsetAsync (the slices that must start at zero) and the two
+ * kernels on the context's stream and calls no cudaMalloc, cudaFree or allocating library routine.  All
+ * pointers are DEVICE pointers owned by the caller, as for dmfe_history_integrals.  Asynchronous.
+ * The array is shared by every call on a device, whatever the context, and keeps the last call's contents:
+ * calls ordered on one stream are safe; calls that overlap on the GPU (two streams without an event between
+ * them, two host threads) race on it and give wrong results.
+ * dmfe_static_init resolves the array's device address for the CURRENT device (which must be the
+ * context's) and clears the array on the context's stream; call it once per device before the first
+ * capture (the first dmfe_history_integrals_static on a device does the same resolution otherwise, which
+ * may load a module).  dmfe_static_limits reports the limits and the array size; any pointer may be NULL. */
+#define DMFE_STATIC_MAX_L 4096
+#define DMFE_STATIC_MAX_ROWS 16384
+DMFE_API int dmfe_static_limits(int32_t *max_L, int32_t *max_rows, int64_t *bytes);
+DMFE_API int dmfe_static_init(dmfe_ctx *ctx);
+DMFE_API int dmfe_history_integrals_static(dmfe_ctx *ctx, const dmfe_grid *grid, const dmfe_rhs_out *out);
 
 /* Device-resident integrator state.  The arrays are caller-owned DEVICE memory.  The device copies of the
  * step size, the row count and the decisions live in the context: a context drives ONE state at a time

@@ -19,6 +19,7 @@ const char *dmfe_strerror(int code) {
     case DMFE_ESTEPMIN: return "step size below h_min";
     case DMFE_ENONFINITE: return "non-finite error estimate";
     case DMFE_ENOMEM: return "out of memory";
+    case DMFE_ETOOLARGE: return "size beyond the static scratch (DMFE_STATIC_MAX_L, DMFE_STATIC_MAX_ROWS)";
     default: return "unknown error";
   }
 }

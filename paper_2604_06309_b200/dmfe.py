@@ -16,9 +16,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdmfe.so")
 
 DMFE_OK, DMFE_EINVAL, DMFE_ECUDA, DMFE_ECAPACITY, DMFE_ESTEPMIN, DMFE_ENONFINITE, DMFE_ENOMEM = 0, -1, -2, -3, -4, -5, -6
+DMFE_ETOOLARGE = -7
+DMFE_STATIC_MAX_L, DMFE_STATIC_MAX_ROWS = 4096, 16384
 
 EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror", "dmfe_get_tables",
-           "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_init_state", "dmfe_rk_step",
+           "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_static_limits", "dmfe_static_init",
+           "dmfe_history_integrals_static", "dmfe_init_state", "dmfe_rk_step",
            "dmfe_advance", "dmfe_dp_step", "dmfe_set_step_size",
            "dmfe_sparsify", "dmfe_integrate", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
            "dmfe_probe_fp64_tflops"]
@@ -92,6 +95,12 @@ def load_library():
     lib.dmfe_get_tables.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_void_p]
     lib.dmfe_history_integrals.restype = c_int
     lib.dmfe_history_integrals.argtypes = [c_void_p, POINTER(dmfe_grid), POINTER(dmfe_rhs_out)]
+    lib.dmfe_static_limits.restype = c_int
+    lib.dmfe_static_limits.argtypes = [POINTER(c_int32), POINTER(c_int32), POINTER(c_int64)]
+    lib.dmfe_static_init.restype = c_int
+    lib.dmfe_static_init.argtypes = [c_void_p]
+    lib.dmfe_history_integrals_static.restype = c_int
+    lib.dmfe_history_integrals_static.argtypes = [c_void_p, POINTER(dmfe_grid), POINTER(dmfe_rhs_out)]
     lib.dmfe_history_integrals_host.restype = c_int
     lib.dmfe_history_integrals_host.argtypes = [c_void_p, c_int32] + [c_void_p] * 7
     lib.dmfe_init_state.restype = c_int
@@ -194,6 +203,28 @@ def dmfe_history_integrals(ctx, n_rows, t, mu, hist, d1C=None, d1R=None, mu_out=
     o = dmfe_rhs_out(d1C=_dev(d1C), d1R=_dev(d1R), mu=_dev(mu_out), d2C=_dev(d2C), d2R=_dev(d2R), F=_dev(F),
                      energy=_dev(energy), sums=_dev(sums), rows1=_dev(rows1), rows2=_dev(rows2))
     _check(lib.dmfe_history_integrals(ctx, byref(g), byref(o)), "dmfe_history_integrals", ctx)
+
+
+def dmfe_static_limits():
+    """(max L, max history rows, bytes of the static scratch array) of dmfe_history_integrals_static."""
+    a, b, c = c_int32(0), c_int32(0), c_int64(0)
+    load_library().dmfe_static_limits(byref(a), byref(b), byref(c))
+    return a.value, b.value, c.value
+
+
+def dmfe_static_init(ctx):
+    _check(load_library().dmfe_static_init(ctx), "dmfe_static_init", ctx)
+
+
+def dmfe_history_integrals_static(ctx, n_rows, t, mu, hist, d1C=None, d1R=None, mu_out=None, d2C=None, d2R=None,
+                                  F=None, energy=None, sums=None, rows1=None, rows2=None):
+    """dmfe_history_integrals without any allocation: per-call tables in the library's static device array
+    (L <= DMFE_STATIC_MAX_L, n_rows - 1 <= DMFE_STATIC_MAX_ROWS, else DMFE_ETOOLARGE); asynchronous."""
+    lib = load_library()
+    g = dmfe_grid(n_rows=n_rows, n_cap=t.shape[0], t=_dev(t), mu=_dev(mu), hist=_dev(hist))
+    o = dmfe_rhs_out(d1C=_dev(d1C), d1R=_dev(d1R), mu=_dev(mu_out), d2C=_dev(d2C), d2R=_dev(d2R), F=_dev(F),
+                     energy=_dev(energy), sums=_dev(sums), rows1=_dev(rows1), rows2=_dev(rows2))
+    _check(lib.dmfe_history_integrals_static(ctx, byref(g), byref(o)), "dmfe_history_integrals_static", ctx)
 
 
 def dmfe_history_integrals_host(ctx, n_rows, t, mu, hist, d1C, d1R, mu_out, energy):
