@@ -190,9 +190,18 @@ typedef struct {
  * error and nothing left to revert (DMFE_ENONFINITE) turns the rest of the batch into no-ops and is
  * returned as the call's code; st and *res describe the state at that point.
  * step_log: optional HOST [n_steps][4] doubles {accepted, eps_RK, h_next, n_rows after} per step.
- * Synchronises on the context's stream. */
+ * Synchronises on the context's stream.
+ * Two implementations of the same arithmetic and decisions (dmfe_set_step_mode): for the 4-point stencil
+ * and L <= 512 the whole batch runs as ONE persistent cooperative kernel (every CTA carries the stage state
+ * in shared memory, a stage costs one grid-wide barrier; csrc/advance_s4.cu); otherwise, or when the device
+ * cannot launch it, as the graph of 21 kernel nodes per step described above.  Sums over the L nodes
+ * (mu, E, eps_RK) are formed in a different order by the two, so their rows agree to rounding, not bit for bit. */
 DMFE_API int dmfe_advance(dmfe_ctx *ctx, dmfe_state *st, int32_t n_steps, int32_t fixed_step,
                           dmfe_advance_result *res, double *step_log);
+
+/* mode 0 (default): dmfe_advance picks the persistent kernel where it applies; mode 1: always the graph of
+ * launches (the path every stencil order and every L takes).  Other values: DMFE_EINVAL. */
+DMFE_API int dmfe_set_step_mode(dmfe_ctx *ctx, int32_t mode);
 
 /* One step: dmfe_advance(ctx, st, 1, fixed_step, ...) with *accepted = the decision. */
 DMFE_API int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *accepted);

@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdmfe.so")
 SOURCES = ["api.cu", "tables.cu", "history_integrals.cu", "pairs_s4.cu", "pairs_generic.cu", "pairs_values.cu", "rk_step.cu", "dp_step.cu",
-           "sparsify.cu", "integrate.cu", "probe.cu", "no_alloc.cu"]
+           "sparsify.cu", "integrate.cu", "probe.cu", "no_alloc.cu", "advance_s4.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 OBJ_DIR = os.path.join(HERE, "build")

@@ -59,6 +59,7 @@ static void free_all(dmfe_ctx *c) {
   if (c->step_exec) cudaGraphExecDestroy(c->step_exec);
   if (c->step_graph) cudaGraphDestroy(c->step_graph);
   cudaFree(c->steplog);
+  cudaFree(c->adv_bar);
   if (c->h_steplog) cudaFreeHost(c->h_steplog);
 }
 

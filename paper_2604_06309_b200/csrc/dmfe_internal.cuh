@@ -104,6 +104,10 @@ struct dmfe_ctx {
   double *steplog;           // [steplog_cap][4] device: {accepted, eps_RK, h_next, n_rows} per step
   double *h_steplog;         // pinned host copy
   int32_t steplog_cap;
+  // a batch of steps as one persistent cooperative kernel (advance_s4.cu)
+  unsigned *adv_bar;  // arrival counter of its grid barrier
+  int adv_off;        // that path is not available on this device / for this size: use the graph of launches
+  int step_mode;      // dmfe_set_step_mode: 0 = automatic, 1 = always the graph of launches
 };
 
 #define CUDA_TRY(ctx, call)                              \
@@ -167,6 +171,8 @@ int dmfe_build_tables(dmfe_ctx *ctx);
 // pairs_values.cu: the right-hand side on a values-only history (dmfe_params.values_only)
 int dmfe_launch_rhs_values(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, const double *mu_hist,
                            const double *hist, const dmfe_rhs_out *out);
+// advance_s4.cu: one batch of SSPRK(10,4) steps as a persistent kernel; 1 = not applicable (take the graph path)
+int dmfe_launch_advance_s4(dmfe_ctx *ctx, dmfe_state *st, int n_steps, int fixed_step, double *log, int log_cap);
 // history_integrals.cu
 // stage: optional stage update run by the pre-pass; deriv_row: optional row of the history whose
 // derivative slots receive F (the derivative is stored with the appended row)

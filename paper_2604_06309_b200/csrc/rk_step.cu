@@ -177,10 +177,18 @@ int dmfe_advance(dmfe_ctx *ctx, dmfe_state *st, int32_t n_steps, int32_t fixed_s
   begin_batch_kernel<<<1, 1, 0, s>>>(ctx->iscal, st->n_rows, ctx->rowtab_dirty);
   ctx->rowtab_dirty = 0;
   CUDA_TRY(ctx, cudaGetLastError());
+  // L <= 512, S = 4: the whole batch as one persistent cooperative kernel (advance_s4.cu)
+  bool persistent = false;
+  {
+    const int rc = dmfe_launch_advance_s4(ctx, st, n_steps, fixed_step, dlog, ctx->steplog_cap);
+    if (rc < 0) return rc;
+    persistent = (rc == DMFE_OK);
+    if (persistent) ctx->rowtab_dirty = 1;  // that kernel keeps the row table its own way
+  }
   // one step as a graph, captured once per (state arrays, mode); plain launches if capture is unavailable
   const void *key[5] = {st->t, st->mu, st->energy, st->hist,
                         (const void *)(uintptr_t)(((uintptr_t)st->n_cap << 2) | (fixed_step ? 1u : 0u) | (dlog ? 2u : 0u))};
-  if (!ctx->graph_off && (ctx->step_exec == nullptr || memcmp(key, ctx->graph_key, sizeof(key)) != 0)) {
+  if (!persistent && !ctx->graph_off && (ctx->step_exec == nullptr || memcmp(key, ctx->graph_key, sizeof(key)) != 0)) {
     if (ctx->step_exec) cudaGraphExecDestroy(ctx->step_exec);
     if (ctx->step_graph) cudaGraphDestroy(ctx->step_graph);
     ctx->step_exec = nullptr;
@@ -202,7 +210,7 @@ int dmfe_advance(dmfe_ctx *ctx, dmfe_state *st, int32_t n_steps, int32_t fixed_s
       memcpy(ctx->graph_key, key, sizeof(key));
     }
   }
-  for (int k = 0; k < n_steps; ++k) {
+  for (int k = 0; k < n_steps && !persistent; ++k) {
     if (ctx->step_exec) {
       CUDA_TRY(ctx, cudaGraphLaunch(ctx->step_exec, s));
     } else {
@@ -234,6 +242,12 @@ int dmfe_advance(dmfe_ctx *ctx, dmfe_state *st, int32_t n_steps, int32_t fixed_s
     res->eps_rk = st->eps_rk;
   }
   return ctx->h_iscal[IS_STATUS];
+}
+
+int dmfe_set_step_mode(dmfe_ctx *ctx, int32_t mode) {
+  if (!ctx || mode < 0 || mode > 1) return DMFE_EINVAL;
+  ctx->step_mode = mode;
+  return DMFE_OK;
 }
 
 int dmfe_rk_step(dmfe_ctx *ctx, dmfe_state *st, int32_t fixed_step, int32_t *accepted) {

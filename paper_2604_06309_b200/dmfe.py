@@ -22,7 +22,7 @@ DMFE_STATIC_MAX_L, DMFE_STATIC_MAX_ROWS = 4096, 16384
 EXPORTS = ["dmfe_create", "dmfe_destroy", "dmfe_last_cuda_error", "dmfe_strerror", "dmfe_get_tables",
            "dmfe_history_integrals", "dmfe_history_integrals_host", "dmfe_static_limits", "dmfe_static_init",
            "dmfe_history_integrals_static", "dmfe_init_state", "dmfe_rk_step",
-           "dmfe_advance", "dmfe_dp_step", "dmfe_set_step_size",
+           "dmfe_advance", "dmfe_set_step_mode", "dmfe_dp_step", "dmfe_set_step_size",
            "dmfe_sparsify", "dmfe_integrate", "dmfe_enable_timing", "dmfe_last_kernel_ms", "dmfe_kernel_time_stats",
            "dmfe_probe_fp64_tflops"]
 
@@ -110,6 +110,8 @@ def load_library():
     lib.dmfe_advance.restype = c_int
     lib.dmfe_advance.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, c_int32, POINTER(dmfe_advance_result),
                                  c_void_p]
+    lib.dmfe_set_step_mode.restype = c_int
+    lib.dmfe_set_step_mode.argtypes = [c_void_p, c_int32]
     lib.dmfe_dp_step.restype = c_int
     lib.dmfe_dp_step.argtypes = [c_void_p, POINTER(dmfe_state), c_int32, POINTER(c_int32)]
     lib.dmfe_set_step_size.restype = c_int
@@ -244,6 +246,11 @@ def make_state(L, n_cap, device="cuda"):
     st = dmfe_state(n_rows=0, n_cap=n_cap, t=_dev(ten["t"]), mu=_dev(ten["mu"]), energy=_dev(ten["energy"]),
                     hist=_dev(ten["hist"]), h=0.0, eps_rk=0.0, n_rhs=0, acc_since=0, startup=0)
     return st, ten
+
+
+def dmfe_set_step_mode(ctx, mode):
+    """0: automatic (persistent kernel for S = 4, L <= 512); 1: always the graph of launches."""
+    _check(load_library().dmfe_set_step_mode(ctx, int(mode)), "dmfe_set_step_mode", ctx)
 
 
 def dmfe_init_state(ctx, st, h0):

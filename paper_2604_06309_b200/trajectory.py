@@ -39,7 +39,7 @@ def observe(theta, t, row, t_w):
 
 def run(L, s, t_max, lam, T, tol, n_cap, t_end, h0=1e-3, sp_every=200, protect_last=24, beta0=0.0,
         t_w=(1e2, 1e3, 1e4, 1e5), n_obs=64, max_steps=None, max_seconds=None, progress=None, startup="ssprk",
-        batch=50, sp_max_passes=8):
+        step_mode=0, batch=50, sp_max_passes=8):
     """Integrate from t = 0 to t_end with the library's step loop (dmfe_integrate: thinning schedule at the
     paper's threshold tol/10, start-up switch, device-resident batches of steps), stopping at log-spaced
     observation times to read one row back.  Returns the observation records, the wall-clock time at which
@@ -48,6 +48,7 @@ def run(L, s, t_max, lam, T, tol, n_cap, t_end, h0=1e-3, sp_every=200, protect_l
     import torch
 
     ctx = D.dmfe_create(L, s, t_max, lam, T=T, beta0=beta0, tol=tol)
+    D.dmfe_set_step_mode(ctx, step_mode)
     rec = dict(t=[], E=[], mu=[], h=[], n_rows=[], corr=[], wall=[])
     out_stats = dict(status="ok")
     milestones = {}
@@ -132,6 +133,8 @@ def main():
     ap.add_argument("--log", default=None, help="append one JSON line per observation record to this file")
     ap.add_argument("--startup", default="ssprk", choices=["ssprk", "dp"],
                     help="dp: Dormand-Prince steps until the stability boundary, then SSPRK(10,4) (PAPER.md:316)")
+    ap.add_argument("--step-mode", type=int, default=0, choices=[0, 1],
+                    help="0: persistent kernel per batch where it applies (S = 4, L <= 512); 1: graph of launches per step")
     args = ap.parse_args()
     cfg = dict(CONFIGS[args.config])
     if args.L:
@@ -151,7 +154,8 @@ def main():
                                         n_rows=rec["n_rows"][-1], corr=rec["corr"][-1], wall=rec["wall"][-1],
                                         steps=int(stats.steps), reverted=int(stats.reverted),
                                         passes=int(stats.sparsify_passes))) + "\n")
-    out = run(t_end=args.t_end, max_seconds=args.max_seconds, progress=progress, startup=args.startup, **cfg)
+    out = run(t_end=args.t_end, max_seconds=args.max_seconds, progress=progress, startup=args.startup,
+              step_mode=args.step_mode, **cfg)
     r = out["records"]
     line = dict(config=args.config, **cfg, t_end=args.t_end, stats=out["stats"], wall_to_t=out["wall_to_t"],
                 E_last=r["E"][-1] if r["E"] else None, corr_last=r["corr"][-1] if r["corr"] else None)

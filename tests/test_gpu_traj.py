@@ -13,11 +13,27 @@ from oracle import dmfe_oracle as O
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def D():
+class _WithStepMode:
+    """The binding with every context switched to one implementation of dmfe_advance (dmfe_set_step_mode):
+    0 = the persistent cooperative kernel where it applies (S = 4, L <= 512), 1 = the graph of launches."""
+
+    def __init__(self, dmfe, mode):
+        self._dmfe, self._mode = dmfe, mode
+
+    def __getattr__(self, name):
+        return getattr(self._dmfe, name)
+
+    def dmfe_create(self, *args, **kw):
+        ctx = self._dmfe.dmfe_create(*args, **kw)
+        self._dmfe.dmfe_set_step_mode(ctx, self._mode)
+        return ctx
+
+
+@pytest.fixture(scope="module", params=[0, 1], ids=["persistent", "graph"])
+def D(request):
     from paper_2604_06309_b200 import dmfe
     dmfe.load_library()
-    return dmfe
+    return _WithStepMode(dmfe, request.param)
 
 
 def _oracle_grid(D, ctx, L, s, t_max):
@@ -376,3 +392,32 @@ def test_trajectory_driver_with_dormand_prince_startup(D):
     # the records are taken at slightly different times: compare through the local slope of E(t)
     slope = (Eb[-1] - Eb[-2]) / (tb[-1] - tb[-2])
     assert abs(Ea[-1] - (Eb[-1] + slope * (ta[-1] - tb[-1]))) < 5e-5
+
+
+def test_step_modes_agree():
+    """The two implementations of dmfe_advance (persistent kernel / graph of launches) on the same run: the same
+    decisions, step sizes bit for bit, rows to rounding (their sums over the nodes run in different orders)."""
+    from paper_2604_06309_b200 import dmfe as D0
+    L, s, lam, T, tol = 512, 4, [0, 0, 0, 1.0], 0.5, 1e-8
+    outs = []
+    for mode in (0, 1):
+        ctx = D0.dmfe_create(L, s, 1e4, lam, T=T, tol=tol)
+        try:
+            D0.dmfe_set_step_mode(ctx, mode)
+            st, ten = D0.make_state(L, 400)
+            D0.dmfe_init_state(ctx, st, 1e-3)
+            logs = []
+            for n in (1, 7, 50, 120, 33):
+                res, log, rc = D0.dmfe_advance(ctx, st, n, want_log=True)
+                assert res.steps == n
+                logs.append(log)
+            outs.append((np.concatenate(logs), st.n_rows, st.h) + _pull(st, ten))
+        finally:
+            D0.dmfe_destroy(ctx)
+    a, b = outs
+    assert a[1] == b[1] and a[2] == b[2]
+    assert np.array_equal(a[0][:, 0], b[0][:, 0]) and np.array_equal(a[0][:, 2:], b[0][:, 2:])   # accept, h_next, rows
+    assert np.array_equal(a[3], b[3])                                                              # t
+    for x, y in zip(a[4:], b[4:]):
+        scale = np.max(np.abs(y), axis=tuple(range(1, y.ndim)), keepdims=True) if y.ndim > 1 else np.abs(y)
+        assert np.all(np.abs(x - y) <= 1e-11 * scale + 1e-300)
