@@ -9,18 +9,32 @@
 //  * The only data a stage exchanges is F (2L doubles): each CTA writes the F_i of its targets, the grid barrier
 //    follows, every CTA reads all of F.  Two F buffers alternate, so that a CTA that runs ahead cannot overwrite
 //    values a slower CTA has not read yet.
-//  * The per-call tables of the pre-pass (packed current row, row brackets, mu weights, jtop, the cubic
-//    coefficient forms of rows M-1 and M) are rebuilt by every CTA in shared memory; the row table lives in
-//    global memory and only grows: entry N = {t_N, 1 / (t_{N+1} - t_N)} is written at the start of the step that
-//    appends row N + 1 (t_{N+1} = t_N + h is known then) and is first read one step later.  The entry of the top
-//    interval [t_{M-1}, t_M] of the stage being evaluated is formed locally (t_M changes with the stage).
+//  * The per-call tables of the pre-pass are rebuilt by every CTA in its shared memory: the packed current row and
+//    its cubic coefficient forms from the state it carries, the forms of row M-1 once per step, the row brackets of
+//    all grid cells, and jtop for its own targets.  Brackets and jtop depend on the stage time and on complete rows
+//    only, so those of stage k + 1 are built between the two halves of the barrier that ends stage k, from the
+//    values of stage k as guesses (one round of independent loads).  The weights of mu(theta_i t_M) are formed
+//    per target in the pair phase.  The row table lives in global memory and only grows: entry
+//    N = {t_N, 1 / (t_{N+1} - t_N)} is written at the start of the step that appends row N + 1 (t_{N+1} = t_N + h
+//    is known then) and is first read one step later.  The entry of the top interval [t_{M-1}, t_M] of the stage
+//    being evaluated is formed locally (t_M changes with the stage).
+//  * Targets are dealt out across the CTAs (CTA b: b, b + #CTAs, ...), so that the expensive targets at small
+//    theta_i (long general loops) do not sit in the same few CTAs.  A thread has at most four pairs per target
+//    here, so every phase of the pair loops of pairs_s4.cuh requests what all of its pairs need before it uses
+//    any of it, and the row searches of a thread's pairs run in lock step.
 //  * CTA 0 alone writes what leaves the kernel: the value slots of the appended row, t[M], the step scalars, the
 //    counters and the optional per-step log.  Nothing it writes is read by another CTA before the next barrier.
+//  * Nothing the kernel itself writes (history, t, mu, row table, F) is read through a read-only (.nc) load.
 //
-// Grid barrier: monotone arrival counter in global memory, release (fence + atomic add) / acquire (ld.acquire
-// spin + fence) by thread 0 of every CTA between two CTA barriers; the kernel is launched cooperatively, so all
-// CTAs are co-resident.  A barrier that is not completed within two seconds makes every CTA leave the kernel
+// Grid barrier: monotone arrival counter in global memory; thread 0 of every CTA arrives with red.release.gpu after
+// a CTA barrier and spins with ld.acquire.gpu before the next CTA barrier; the kernel is launched cooperatively, so
+// all CTAs are co-resident.  A barrier that is not completed within two seconds makes every CTA leave the kernel
 // with status DMFE_ECUDA instead of hanging the device.
+//
+// Measured on B200 at the shape of BASELINE.json config 4 (L = 512, 128 CTAs x 512 threads, 139 KB of shared
+// memory): ~32 k clk = 16 us per stage (pair phase 20 k, update + reductions 5 k, tables behind the barrier 3.5 k,
+// barrier 1.5 - 3 k) against 22 us for the two launches of the graph path; the pair phase is bound by the L1 data
+// path like the full-size kernel, growing to 27 k clk at 20 k rows.
 #include <math.h>
 #include <string.h>
 
@@ -68,29 +82,33 @@ __device__ __forceinline__ unsigned long long global_ns() {
   return v;
 }
 
-// all CTAs of the (cooperative) grid; returns false when the barrier timed out
-__device__ __forceinline__ bool grid_sync(unsigned *ctr, unsigned &target, unsigned nb, int *s_fail) {
+// Grid barrier of the (cooperative) grid in two halves, so that work that needs nothing from the other CTAs can
+// run between them: grid_arrive publishes this CTA's writes, grid_wait returns once every CTA has arrived (false
+// when that did not happen within two seconds).
+__device__ __forceinline__ void grid_arrive(unsigned *ctr, unsigned &target, unsigned nb) {
   __syncthreads();
   target += nb;
+  if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(ctr) : "memory");
+}
+__device__ __forceinline__ bool grid_wait(unsigned *ctr, unsigned target, int *s_fail) {
   if (threadIdx.x == 0) {
-    __threadfence();
-    atomicAdd(ctr, 1u);
     const unsigned long long t0 = global_ns();
-    int fail = 0;
     for (;;) {
       unsigned v;
       asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
       if (v >= target) break;
       if (global_ns() - t0 > 2000000000ull) {
-        fail = 1;
+        *s_fail = 1;
         break;
       }
     }
-    __threadfence();
-    if (fail) *s_fail = 1;
   }
   __syncthreads();
   return *s_fail == 0;
+}
+__device__ __forceinline__ bool grid_sync(unsigned *ctr, unsigned &target, unsigned nb, int *s_fail) {
+  grid_arrive(ctr, target, nb);
+  return grid_wait(ctr, target, s_fail);
 }
 
 // n = max{ n in [0, top] : t[n] <= tau } from a guess g (rhs_common.cuh: row_search_from; here without the
@@ -142,8 +160,8 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
   __shared__ int s_fail;
   const int L = a.L;
   double2 *s_q1 = reinterpret_cast<double2 *>(smem_dyn), *s_q2 = s_q1 + L, *s_dl = s_q2 + L;
-  double2 *s_cur = s_dl + L, *s_muw = s_cur + L;
-  double4 *s_coefM = reinterpret_cast<double4 *>(s_muw + L);  // [L][2]
+  double2 *s_cur = s_dl + L;
+  double4 *s_coefM = reinterpret_cast<double4 *>(s_cur + L);  // [L][2]
   double4 *s_coefT = s_coefM + 2 * (size_t)L;                 // [L][4]
   int2 *s_br = reinterpret_cast<int2 *>(s_coefT + 4 * (size_t)L);
   int32_t *s_blo = reinterpret_cast<int32_t *>(s_br + L), *s_jtop = s_blo + L;
@@ -163,7 +181,7 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
   unsigned bar_target = 0;
   int parity = 0;
   if (tid == 0) s_fail = 0;
-  if (tid < L) s_blo[tid] = 0;
+  for (int c = tid; c < L; c += ADV_THREADS) s_blo[c] = 0, s_jtop[c] = 0;
 
   int rows = a.iscal[IS_NROWS];  // complete rows = index M of the row a step appends
   double h_next = a.scal[SC_HNEXT];
@@ -196,8 +214,70 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
       o[2] = cubic_form(y0.z, y1.z, y2.z, y3.z);
       o[3] = cubic_form(y0.w, y1.w, y2.w, y3.w);
     }
+    // ---- per-call tables of a stage time tM, every CTA its own copy in shared memory.  They depend on the stage
+    // time and on complete rows only, so the tables of stage k + 1 are built between the two halves of the grid
+    // barrier that ends stage k.  (1) All nodes c: blo[c] = n(theta_c t_M) and the row brackets br of the grid cells
+    // (every target's general pairs use them); the value of the previous stage is the guess: successive stage
+    // times differ by a fraction of a step, so n is the guess or a neighbour, decided by one round of four
+    // independent loads.  (2) Only for the targets of this CTA: jtop[i], by the first warp of the target's group
+    // (the weights of mu(theta_i t_M) are formed in the pair phase, behind the loads of the type-1 half) ----
+    auto build_tables = [&](const double tM) {
+      const int top = M - 1;
+      for (int c = tid; c < L; c += ADV_THREADS) {
+        const double tau1 = __dmul_rn(a.theta[c], tM);
+        const int g = min(max(s_blo[c], 0), top);
+        const double ta = (g >= 1) ? a.t[g - 1] : -INFINITY, tb = a.t[g];
+        const double tc = (g + 1 <= top) ? a.t[g + 1] : INFINITY, td = (g + 2 <= top) ? a.t[g + 2] : INFINITY;
+        int n;
+        if (ta <= tau1 && tau1 < td) {
+          n = (tc <= tau1) ? g + 1 : ((tb <= tau1) ? g : g - 1);
+        } else {  // far guess (first stage after a thinning or a revert)
+          n = row_search_hint(a.t, top, g, tau1);
+        }
+        s_blo[c] = n;
+        // row bracket of the grid cell of phi2 by stencil start (history_integrals.cu: PrepS4::br)
+        if (c >= 2 && c <= L - 3) s_br[c - 1].x = n;
+        if (c >= 2 && c <= L - 3) s_br[c - 2].y = n;
+        if (c == 0) s_br[0].x = n;
+        if (c == L - 1) s_br[L - 4].y = n;
+      }
+      __syncthreads();
+      if (wg == 0) {
+        for (int i = group * (int)nb + blockIdx.x; i < L; i += (int)nb * ngroups) {
+          const double th_i = a.theta[i], om_i = a.omega[i];
+          const double tau1 = __dmul_rn(th_i, tM);
+          {
+            // jtop[i]: first node j whose type-2 lookup falls into the top interval [t_{M-1}, t_M):
+            // tau2(i, j) = fl(fl(theta_i + fl(omega_i theta_j)) t_M) is monotone in j.  The lanes test the 32 nodes
+            // around the previous stage's value; nodes past the end count as inside
+            auto in_top = [&](int j) { return __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, a.theta[j])), tM) >= t0; };
+            const int gj = min(max(s_jtop[i], 0), L);
+            const int j0 = gj - 16, jq = j0 + lane;
+            const bool in_l = (jq >= L) || (jq >= 0 && in_top(jq));
+            const unsigned mask = __ballot_sync(0xffffffffu, in_l);
+            int jt;
+            if ((mask >> 31) && (j0 <= 0 || !(mask & 1u))) {
+              jt = min(j0 + (__ffs(mask) - 1), L);
+            } else {
+              int lo = 0, hi = L;
+              if (mask >> 31) hi = max(j0, 0); else lo = min(j0 + 32, L);
+              while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (in_top(mid))
+                  hi = mid;
+                else
+                  lo = mid + 1;
+              }
+              jt = lo;
+            }
+            if (lane == 0) s_jtop[i] = jt;
+          }
+        }
+      }
+    };
     int accept = 1;
     double hn = h, eps_step = 0.0;
+    build_tables(__dadd_rn(t0, __dmul_rn(a_stage_c[1], h)));  // stage 0
 
     for (int k = 0; k < 10 && status == 0; ++k) {
       const double tM = (k < 9) ? __dadd_rn(t0, __dmul_rn(a_stage_c[k + 1], h)) : tNext;
@@ -243,7 +323,7 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
           cell[2] = qa.y;
         }
         if (l == 0) s_c0 = qa.x;
-        const double fp = horner(mc.c1, mc.pmax - 1, qa.x), fpp = horner(mc.c2, mc.pmax - 2, qa.x);
+        const double fp = f1<PD>(mc, qa.x), fpp = f2<PD>(mc, qa.x);
         const double nj = a.nu[l];
         am += nj * (fpp * qa.y * qa.x + fp * qa.y);
         ae += nj * (fp * qa.y);
@@ -255,12 +335,21 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
       }
       if (lane == 0) s_part[0][warp] = am, s_part[1][warp] = ae, s_part[2][warp] = eacc;
       __syncthreads();  // also: s_cur, s_q* complete
-      double tm = 0.0, te = 0.0, eps = 0.0;
+      // the 16 warp sums, added in the same butterfly order by every warp of every CTA
+      double tm = s_part[0][lane & (ADV_WARPS - 1)], te = s_part[1][lane & (ADV_WARPS - 1)];
+      double eps = s_part[2][lane & (ADV_WARPS - 1)];
 #pragma unroll
-      for (int w = 0; w < ADV_WARPS; ++w) tm += s_part[0][w], te += s_part[1][w], eps += s_part[2][w];
+      for (int o = ADV_WARPS / 2; o > 0; o >>= 1) {
+        tm += __shfl_xor_sync(0xffffffffu, tm, o);
+        te += __shfl_xor_sync(0xffffffffu, te, o);
+        eps += __shfl_xor_sync(0xffffffffu, eps, o);
+      }
       const double c0 = s_c0;
-      const double mu = mc.T + tM * tm + mc.beta0 * horner(mc.c1, mc.pmax - 1, c0) * c0;  // Eq.(13)
-      const double E = -tM * te - mc.beta0 * horner(mc.c0, mc.pmax, c0);                   // Eq.(14)
+      double mu = mc.T + tM * tm, E = -tM * te;  // Eq.(13), Eq.(14)
+      if (mc.beta0 != 0.0) {
+        mu += mc.beta0 * f1<PD>(mc, c0) * c0;
+        E -= mc.beta0 * horner(mc.c0, mc.pmax, c0);
+      }
       if (k == 9) {  // eps_RK (Eq.(25)) and the controller (reading G20)
         eps_step = eps;
         if (!a.fixed_step) {
@@ -287,52 +376,6 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
           a.iscal[IS_ACCEPT] = accept;
         }
       }
-      // ---- per-call tables of this stage time, every CTA its own copy in shared memory ----
-      for (int c = tid; c < L; c += ADV_THREADS) {
-        const double tau1 = __dmul_rn(a.theta[c], tM);
-        const int n = row_search_hint(a.t, M - 1, s_blo[c], tau1);
-        s_blo[c] = n;
-        {
-          // mu(theta_c t_M): local 4-point Lagrange in t over rows k0..k0+3 (reading G11); the weight of the
-          // current row's mu is kept apart (history_integrals.cu)
-          const int npts = (M + 1 < 4) ? M + 1 : 4;
-          int k0 = n - 1;
-          if (k0 > M + 1 - npts) k0 = M + 1 - npts;
-          if (k0 < 0) k0 = 0;
-          double tq[4];
-          for (int q = 0; q < npts; ++q) tq[q] = (k0 + q == M) ? tM : a.t[k0 + q];
-          double part = 0.0, wM = 0.0;
-          for (int p = 0; p < npts; ++p) {
-            double wgt = 1.0;
-            for (int q = 0; q < npts; ++q)
-              if (q != p) wgt *= (tau1 - tq[q]) / (tq[p] - tq[q]);
-            if (k0 + p == M)
-              wM = wgt;
-            else
-              part += wgt * a.mu[k0 + p];
-          }
-          s_muw[c] = make_double2(part, wM);
-        }
-        // row bracket of the grid cell of phi2 by stencil start (history_integrals.cu: PrepS4::br)
-        if (c >= 2 && c <= L - 3) s_br[c - 1].x = n;
-        if (c >= 2 && c <= L - 3) s_br[c - 2].y = n;
-        if (c == 0) s_br[0].x = n;
-        if (c == L - 1) s_br[L - 4].y = n;
-        {
-          // first node j of target c whose type-2 lookup falls into the top interval [t_{M-1}, t_M)
-          const double th_i = a.theta[c], om_i = a.omega[c];
-          int lo = 0, hi = L;
-          while (lo < hi) {
-            const int mid = (lo + hi) >> 1;
-            const double tau2 = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, a.theta[mid])), tM);
-            if (tau2 >= t0)
-              hi = mid;
-            else
-              lo = mid + 1;
-          }
-          s_jtop[c] = lo;
-        }
-      }
       for (int s0 = tid; s0 < L - 3; s0 += ADV_THREADS) {  // cubic forms of the row just formed
         const double2 y0 = s_cur[s0], y1 = s_cur[s0 + 1], y2 = s_cur[s0 + 2], y3 = s_cur[s0 + 3];
         s_coefM[2 * (size_t)s0] = cubic_form(y0.x, y1.x, y2.x, y3.x);
@@ -343,7 +386,9 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
       double2 *Fout = a.Fbuf + (size_t)((k + 1) & 1) * L;
 
       // ---- the L^2 pairs (pairs_s4.cuh: same loops, tables in shared memory) ----
-      for (int i = blockIdx.x * ngroups + group; i < L; i += (int)nb * ngroups, parity ^= 1) {
+      // targets are dealt out across the CTAs (CTA b: b, b + nb, b + 2 nb, ...): the expensive small-theta targets
+      // (long general loops) are spread over all SMs instead of sitting in the first few CTAs
+      for (int i = group * (int)nb + blockIdx.x; i < L; i += (int)nb * ngroups, parity ^= 1) {
         const double th_i = a.theta[i], om_i = a.omega[i];
         const double tau1 = __dmul_rn(th_i, tM);
         const int n1 = s_blo[i];
@@ -353,58 +398,72 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
           const double2 rt = top1 ? rtT : rowtab[n1];
           t_weights(rt.x, rt.y, tau1, top1, h1);
         }
+        // A thread has K <= KMAX = 4 pairs per target here (L <= 512, at least four warps per target), so the
+        // loops of pairs_s4.cuh, which keep one pair in flight, would pay a memory round trip per pair.  Instead
+        // every phase requests what all of the thread's pairs need before it uses any of it.
+        constexpr int KMAX = 4;
+        double2 mw = make_double2(0.0, 0.0);  // weights of mu(theta_i t_M); used by the group's first thread
+        const uint64_t *pt1 = a.tab + (size_t)i * (size_t)L + tig;
+        const uint64_t *pt2 = pt1 + plane, *pt3 = pt2 + plane;
         // ================= type-1 half of Eq.(21): S1, S3, S5, S6 =================
-        auto type1 = [&](auto top1_c) {
-          constexpr bool TOP1 = decltype(top1_c)::value;
-          double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
-          const uint64_t *pt = a.tab + (size_t)i * (size_t)L + tig;
+        {
+          uint64_t e1[KMAX];
+          double nu1[KMAX];
+          double4 lo1[KMAX], hi1[KMAX];
           const double4 *pc = hist + (size_t)n1 * (size_t)L + tig;
-          const double *pn = a.nu + tig;
-          const double2 *pu = s_cur + tig;
-          uint64_t e_c = 0, e_n = 0;
-          double nu_c = 0.0;
-          double4 lo_c = make_double4(0, 0, 0, 0), hi_c = lo_c;
-          if (K > 0) {
-            e_c = ld_stream(pt);
-            nu_c = *pn;
-            lo_c = ld_cell(pc);
-            if (TOP1) {
-              const double2 c = *pu;
-              hi_c = make_double4(c.x, 0.0, c.y, 0.0);
-            } else {
-              hi_c = ld_cell(pc + L);
-            }
-          }
-          if (K > 1) e_n = ld_stream(pt + TG);
-#pragma unroll 2
-          for (int kk = 0; kk < K; ++kk) {
-            uint64_t e_nn = 0;
-            double nu_n = 0.0;
-            double4 lo_n = make_double4(0, 0, 0, 0), hi_n = lo_n;
-            pt += TG, pc += TG, pn += TG, pu += TG;
-            if (kk + 2 < K) e_nn = ld_stream(pt + TG);
-            if (kk + 1 < K) {
-              nu_n = *pn;
-              lo_n = ld_cell(pc);
-              if (TOP1) {
-                const double2 c = *pu;
-                hi_n = make_double4(c.x, 0.0, c.y, 0.0);
+#pragma unroll
+          for (int q = 0; q < KMAX; ++q) {
+            e1[q] = 0, nu1[q] = 0.0;
+            lo1[q] = hi1[q] = make_double4(0.0, 0.0, 0.0, 0.0);
+            if (q < K) {
+              e1[q] = ld_stream(pt1 + q * TG);
+              nu1[q] = a.nu[tig + q * TG];
+              lo1[q] = ld_cell(pc + q * TG);
+              if (top1) {  // upper row = the current row: values only (reading G12)
+                const double2 c = s_cur[tig + q * TG];
+                hi1[q] = make_double4(c.x, 0.0, c.y, 0.0);
               } else {
-                hi_n = ld_cell(pc + L);
+                hi1[q] = ld_cell(pc + L + q * TG);
               }
             }
-            const double2 A1 = a_factor(s_cur, e_c);
-            const double C1 = A1.x, R1 = A1.y;
-            const double B1C = TOP1 ? h1[0] * lo_c.x + h1[1] * lo_c.y + h1[2] * hi_c.x
-                                    : h1[0] * lo_c.x + h1[1] * lo_c.y + h1[2] * hi_c.x + h1[3] * hi_c.y;
-            const double B1R = TOP1 ? h1[0] * lo_c.z + h1[1] * lo_c.w + h1[2] * hi_c.z
-                                    : h1[0] * lo_c.z + h1[1] * lo_c.w + h1[2] * hi_c.z + h1[3] * hi_c.w;
-            const double nR1 = nu_c * R1, nB1R = nu_c * B1R;
-            acc0 = fma(f2<PD>(mc, C1) * nR1, B1C, acc0);   // S1
-            acc1 = fma(f1<PD>(mc, C1), nB1R, acc1);        // S3
-            acc2 = fma(f2<PD>(mc, B1C) * nB1R, C1, acc2);  // S5
-            acc3 = fma(f1<PD>(mc, B1C), nR1, acc3);        // S6
-            e_c = e_n, e_n = e_nn, nu_c = nu_n, lo_c = lo_n, hi_c = hi_n;
+          }
+          if (wg == 0) {
+            // mu(theta_i t_M) = mw.x + mw.y mu(t_M): local 4-point Lagrange in t over rows k0..k0+3 (reading G11),
+            // lane p holds point p, the weight of the current row's mu kept apart; its loads travel with the
+            // type-1 loads above.  w_p = prod_{q != p} (tau - t_q) / prod_{q != p} (t_p - t_q)
+            const int npts = (M + 1 < 4) ? M + 1 : 4;
+            const int k0 = min(max(n1 - 1, 0), M + 1 - npts);
+            const bool stored = lane < npts && k0 + lane < M;
+            const double tq_l = stored ? a.t[k0 + lane] : tM, mq_l = stored ? a.mu[k0 + lane] : 0.0;
+            double num = 1.0, den = 1.0;
+            for (int q = 0; q < npts; ++q) {
+              const double tq = __shfl_sync(0xffffffffu, tq_l, q);
+              if (q != lane) num *= (tau1 - tq), den *= (tq_l - tq);
+            }
+            const double wgt = num / den;
+            const bool is_cur = (k0 + lane == M);
+            const double part_l = (lane < npts && !is_cur) ? wgt * mq_l : 0.0, wM_l = (lane < npts && is_cur) ? wgt : 0.0;
+            double part = 0.0, wM = 0.0;
+            for (int q = 0; q < npts; ++q) {  // points in order, as a sequential sum
+              part += __shfl_sync(0xffffffffu, part_l, q);
+              wM += __shfl_sync(0xffffffffu, wM_l, q);
+            }
+            mw = make_double2(part, wM);
+          }
+          double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+#pragma unroll
+          for (int q = 0; q < KMAX; ++q) {
+            if (q < K) {
+              const double2 A1 = a_factor(s_cur, e1[q]);
+              const double C1 = A1.x, R1 = A1.y;
+              const double B1C = h1[0] * lo1[q].x + h1[1] * lo1[q].y + h1[2] * hi1[q].x + h1[3] * hi1[q].y;
+              const double B1R = h1[0] * lo1[q].z + h1[1] * lo1[q].w + h1[2] * hi1[q].z + h1[3] * hi1[q].w;
+              const double nR1 = nu1[q] * R1, nB1R = nu1[q] * B1R;
+              acc0 = fma(f2<PD>(mc, C1) * nR1, B1C, acc0);   // S1: K(t,s) C(t',s)
+              acc1 = fma(f1<PD>(mc, C1), nB1R, acc1);        // S3: D(t,s) R(t',s)
+              acc2 = fma(f2<PD>(mc, B1C) * nB1R, C1, acc2);  // S5: K(t',s) C(t,s)
+              acc3 = fma(f1<PD>(mc, B1C), nR1, acc3);        // S6: D(t',s) R(t,s)
+            }
           }
           const double acc[4] = {acc0, acc1, acc2, acc3};
           constexpr int slot[4] = {0, 2, 4, 5};
@@ -414,80 +473,87 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
             if (lane == 0) red[parity][warp][slot[q]] = v;
           }
-        };
-        const int jt = s_jtop[i];
-        const uint64_t *pt2 = a.tab + plane + (size_t)i * (size_t)L + tig;
-        const uint64_t *pt3 = pt2 + plane;
-        const double2 *pn = a.thnu + tig;
-        uint64_t e2_c = 0, e3_c = 0, e2_n = 0, e3_n = 0;
-        double2 tn_c = make_double2(0.0, 0.0), tn_n = tn_c;
-        if (K > 0) {
-          e2_c = ld_stream(pt2);
-          e3_c = ld_stream(pt3);
-          tn_c = *pn;
         }
-        if (K > 1) {
-          e2_n = ld_stream(pt2 + TG);
-          e3_n = ld_stream(pt3 + TG);
-          tn_n = pn[TG];
-        }
-        if (top1)
-          type1(std::true_type{});
-        else
-          type1(std::false_type{});
-
         // ================= type-2 half: S2, S4, S7, S8 =================
         {
-          double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+          const int jt = s_jtop[i];
           int Kg = (jt > tig) ? (jt - tig + TG - 1) / TG : 0;  // this thread's pairs with j < jtop[i]
           if (Kg > K) Kg = K;
+          uint64_t e2[KMAX], e3[KMAX];
+          double2 tn[KMAX];
+          double tau2[KMAX];
+#pragma unroll
+          for (int q = 0; q < KMAX; ++q) {
+            e2[q] = e3[q] = 0;
+            tn[q] = make_double2(0.0, 0.0);
+            if (q < K) {
+              e2[q] = ld_stream(pt2 + q * TG);
+              e3[q] = ld_stream(pt3 + q * TG);
+              tn[q] = a.thnu[tig + q * TG];
+            }
+          }
+#pragma unroll
+          for (int q = 0; q < KMAX; ++q) tau2[q] = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn[q].x)), tM);
+          // ---- index stage of the general pairs (j < jtop[i]: n2 <= M - 2, both rows complete): n2 =
+          // max{n in [lo, hi] : t_n <= tau2} by bisection inside the bracket br[a2], the thread's
+          // pairs in lock step so that the row-table loads of one round are independent ----
+          int lo2[KMAX], hi2[KMAX];
+          double2 rt2[KMAX];
+#pragma unroll
+          for (int q = 0; q < KMAX; ++q) {
+            lo2[q] = hi2[q] = 0;
+            rt2[q] = make_double2(0.0, 1.0);
+            if (q < Kg) {
+              const int2 b = s_br[tab_start(e2[q])];
+              lo2[q] = b.x;
+              hi2[q] = min(b.y, M - 2);
+              rt2[q] = rowtab[b.x];
+            }
+          }
+          for (bool more = true; more;) {
+            more = false;
+            int mid[KMAX];
+            double2 rm[KMAX];
+#pragma unroll
+            for (int q = 0; q < KMAX; ++q) {
+              mid[q] = lo2[q] + ((hi2[q] - lo2[q] + 1) >> 1);
+              rm[q] = rt2[q];
+              if (lo2[q] < hi2[q]) rm[q] = rowtab[mid[q]];
+            }
+#pragma unroll
+            for (int q = 0; q < KMAX; ++q) {
+              if (lo2[q] < hi2[q]) {
+                if (rm[q].x <= tau2[q])
+                  lo2[q] = mid[q], rt2[q] = rm[q];
+                else
+                  hi2[q] = mid[q] - 1;
+                more |= (lo2[q] < hi2[q]);
+              }
+            }
+          }
+          double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
           auto finish = [&](double nj, double C2, double R2, double B2C, double B2R) {
             const double nR2 = nj * R2;
             const double K2 = f2<PD>(mc, C2) * nR2;
-            acc0 = fma(K2, B2C, acc0);                     // S2
-            acc1 = fma(K2, B2R, acc1);                     // S4
-            acc2 = fma(f1<PD>(mc, B2C), nR2, acc2);        // S7
-            acc3 = fma(nR2, f2<PD>(mc, B2C) * B2R, acc3);  // S8
+            acc0 = fma(K2, B2C, acc0);                     // S2: K(t,s) C(s,t')
+            acc1 = fma(K2, B2R, acc1);                     // S4: K(t,s) R(s,t')
+            acc2 = fma(f1<PD>(mc, B2C), nR2, acc2);        // S7: D(s,t') R(t,s)
+            acc3 = fma(nR2, f2<PD>(mc, B2C) * B2R, acc3);  // S8: R(t,s) K(s,t')
           };
-          int kk = 0;
-          // general pairs (n2 <= M - 2: both rows complete, row-table entries final)
-          if (Kg > 0) {
-            int n2_c;
-            double tau2_c;
-            double2 rt_c;
-            {
-              tau2_c = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn_c.x)), tM);
-              const int2 b = s_br[tab_start(e2_c)];
-              n2_c = probe_row(rowtab, b.x, min(b.y, M - 2), tau2_c);
-              rt_c = rowtab[n2_c];
-            }
-#pragma unroll 2
-            for (; kk < Kg; ++kk) {
-              const int a3 = tab_start(e3_c);
-              const double4 *p2 = hist + ((size_t)n2_c * (size_t)L + (size_t)a3);
-              double4 x[4];
+          // ---- general pairs: theta-stencil on the cells of rows n2 and n2 + 1, cubic Hermite in t (Eq.(20)) ----
+#pragma unroll
+          for (int q = 0; q < KMAX; ++q) {
+            if (q < Kg) {
+              const int a3 = tab_start(e3[q]);
+              const double4 *p2 = hist + ((size_t)lo2[q] * (size_t)L + (size_t)a3);
+              double4 x[4], y[4];
 #pragma unroll
               for (int l = 0; l < 4; ++l) x[l] = ld_cell(p2 + l);
-              int n2_n = 0;
-              double tau2_n = 0.0;
-              double2 rt_n = make_double2(0.0, 0.0);
-              if (kk + 1 < Kg) {
-                tau2_n = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn_n.x)), tM);
-                const int2 b = s_br[tab_start(e2_n)];
-                n2_n = probe_row(rowtab, b.x, min(b.y, M - 2), tau2_n);
-                rt_n = rowtab[n2_n];
-              }
-              uint64_t e2_nn = 0, e3_nn = 0;
-              double2 tn_nn = make_double2(0.0, 0.0);
-              pt2 += TG, pt3 += TG, pn += TG;
-              if (kk + 2 < K) {
-                e2_nn = ld_stream(pt2 + TG);
-                e3_nn = ld_stream(pt3 + TG);
-                tn_nn = pn[TG];
-              }
-              const double v3 = tab_v(e3_c);
+#pragma unroll
+              for (int l = 0; l < 4; ++l) y[l] = ld_cell(p2 + L + l);
+              const double v3 = tab_v(e3[q]);
               double h2[4];
-              t_weights(rt_c.x, rt_c.y, tau2_c, false, h2);
+              t_weights(rt2[q].x, rt2[q].y, tau2[q], false, h2);
               double w[4];
               lagrange4_centred(v3, w);
               double cl = 0.0, dcl = 0.0, rl = 0.0, drl = 0.0, cu = 0.0, dcu = 0.0, ru = 0.0, dru = 0.0;
@@ -500,56 +566,36 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
               }
 #pragma unroll
               for (int l = 0; l < 4; ++l) {
-                const double4 y = ld_cell(p2 + L + l);
-                cu = fma(w[l], y.x, cu);
-                dcu = fma(w[l], y.y, dcu);
-                ru = fma(w[l], y.z, ru);
-                dru = fma(w[l], y.w, dru);
+                cu = fma(w[l], y[l].x, cu);
+                dcu = fma(w[l], y[l].y, dcu);
+                ru = fma(w[l], y[l].z, ru);
+                dru = fma(w[l], y[l].w, dru);
               }
-              const double2 A2 = a_factor(s_cur, e2_c);
+              const double2 A2 = a_factor(s_cur, e2[q]);
               const double B2C = h2[0] * cl + h2[1] * dcl + h2[2] * cu + h2[3] * dcu;
               const double B2R = h2[0] * rl + h2[1] * drl + h2[2] * ru + h2[3] * dru;
-              finish(tn_c.y, A2.x, A2.y, B2C, B2R);
-              e2_c = e2_n, e3_c = e3_n, tn_c = tn_n;
-              e2_n = e2_nn, e3_n = e3_nn, tn_n = tn_nn;
-              n2_c = n2_n, tau2_c = tau2_n, rt_c = rt_n;
+              finish(tn[q].y, A2.x, A2.y, B2C, B2R);
             }
           }
-          // top pairs (n2 = M - 1): rows M-1 and M through their coefficient forms, quadratic in t (G12)
-          {
-            int a3_held = -1;
-            double4 qc = make_double4(0, 0, 0, 0), qdc = qc, qr = qc, qdr = qc, uc = qc, ur = qc;
-#pragma unroll 2
-            for (; kk < K; ++kk) {
-              const int a3 = tab_start(e3_c);
-              if (a3 != a3_held) {
-                qc = s_coefT[4 * a3], qdc = s_coefT[4 * a3 + 1];
-                qr = s_coefT[4 * a3 + 2], qdr = s_coefT[4 * a3 + 3];
-                uc = s_coefM[2 * a3], ur = s_coefM[2 * a3 + 1];
-                a3_held = a3;
-              }
-              const double v3 = tab_v(e3_c);
-              const double2 A2 = a_factor(s_cur, e2_c);
-              const double2 tn = tn_c;
-              uint64_t e2_nn = 0, e3_nn = 0;
-              double2 tn_nn = make_double2(0.0, 0.0);
-              pt2 += TG, pt3 += TG, pn += TG;
-              if (kk + 2 < K) {
-                e2_nn = ld_stream(pt2 + TG);
-                e3_nn = ld_stream(pt3 + TG);
-                tn_nn = pn[TG];
-              }
-              const double tau2 = __dmul_rn(__dadd_rn(th_i, __dmul_rn(om_i, tn.x)), tM);
-              const double d = tau2 - rtT.x;
+          // ---- top pairs (j >= jtop[i]: n2 = M - 1): rows M-1 and M through their coefficient forms, quadratic
+          // in t (reading G12): B = (1 - u^2) Y_{M-1} + d (1 - u) Y'_{M-1} + u^2 Y_M ----
+#pragma unroll
+          for (int q = 0; q < KMAX; ++q) {
+            if (q >= Kg && q < K) {
+              const int a3 = tab_start(e3[q]);
+              const double4 qc = s_coefT[4 * a3], qdc = s_coefT[4 * a3 + 1];
+              const double4 qr = s_coefT[4 * a3 + 2], qdr = s_coefT[4 * a3 + 3];
+              const double4 uc = s_coefM[2 * a3], ur = s_coefM[2 * a3 + 1];
+              const double v3 = tab_v(e3[q]);
+              const double2 A2 = a_factor(s_cur, e2[q]);
+              const double d = tau2[q] - rtT.x;
               const double u = d * rtT.y;
               const double q2 = u * u;
               const double q0 = 1.0 - q2;
               const double q1 = d * (1.0 - u);
               const double B2C = fma(q0, cubic(qc, v3), fma(q1, cubic(qdc, v3), q2 * cubic(uc, v3)));
               const double B2R = fma(q0, cubic(qr, v3), fma(q1, cubic(qdr, v3), q2 * cubic(ur, v3)));
-              finish(tn.y, A2.x, A2.y, B2C, B2R);
-              e2_c = e2_n, e3_c = e3_n, tn_c = tn_n;
-              e2_n = e2_nn, e3_n = e3_nn, tn_n = tn_nn;
+              finish(tn[q].y, A2.x, A2.y, B2C, B2R);
             }
           }
           const double acc[4] = {acc0, acc1, acc2, acc3};
@@ -582,7 +628,6 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
             if (!top1) hi = ld_cell(hist + (size_t)(n1 + 1) * (size_t)L);
             b1c_first = h1[0] * lo.x + h1[1] * lo.y + h1[2] * hi.x + h1[3] * hi.y;
           }
-          const double2 mw = s_muw[i];
           const double mu_p = fma(mw.y, mu, mw.x);
           const double2 ci = s_cur[i], cz = s_cur[0];
           const double fc = mc.beta0 * f1<PD>(mc, cz.x) * b1c_first;
@@ -604,7 +649,9 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
           }
         }
       }
-      if (!grid_sync(a.bar, bar_target, nb, &s_fail)) status = DMFE_ECUDA;
+      grid_arrive(a.bar, bar_target, nb);
+      if (k < 9) build_tables((k + 1 < 9) ? __dadd_rn(t0, __dmul_rn(a_stage_c[k + 2], h)) : tNext);
+      if (!grid_wait(a.bar, bar_target, &s_fail)) status = DMFE_ECUDA;
     }  // stages
     if (status != 0) break;
     // ---- commit (rk_step.cu: commit_step_kernel), identical in every CTA ----
@@ -677,10 +724,12 @@ int dmfe_launch_advance_s4(dmfe_ctx *ctx, dmfe_state *st, int n_steps, int fixed
       if (eff >= 0.97) break;
     }
   }
+  while (G < ADV_WARPS && L > 4 * 32 * G) G *= 2;  // the kernel's pair phase holds at most 4 pairs per thread
+  if (L > 4 * 32 * G) return 1;
   const int ngroups = ADV_WARPS / G;
   int grid = (L + ngroups - 1) / ngroups;
   if (grid > ctx->sm_count) grid = ctx->sm_count;
-  const size_t smem = 288 * (size_t)L;
+  const size_t smem = 272 * (size_t)L;  // q1, q2, delta, cur: 4 x 16 L; coefM 64 L, coefT 128 L; br 8 L, blo + jtop 8 L
   if (smem > (size_t)ctx->smem_max) return 1;
   AdvArgs a;
   memset(&a, 0, sizeof(a));
