@@ -444,7 +444,7 @@ def run_ours(args):
     if args.traj_seconds > 0:
         from paper_2604_06309_b200 import trajectory
         cfg = dict(trajectory.CONFIGS[4])
-        out = trajectory.run(t_end=1e7, max_seconds=args.traj_seconds, **cfg)
+        out = trajectory.run(t_end=1e7, max_seconds=args.traj_seconds, step_mode=args.step_mode, **cfg)
         stt = out["stats"]
         traj = {"workload": "config4: pure 3-spin aging run, T=0.5, tol=1e-8, L=%d, s=%d, n_cap=%d, first %.0f s of "
                             "wall time" % (cfg["L"], cfg["s"], cfg["n_cap"], args.traj_seconds),
@@ -454,7 +454,9 @@ def run_ours(args):
                 "sparsify_passes": stt["sparsify_passes"], "rows_dropped": stt["rows_dropped"],
                 "eps_sparse_over_tol": stt["eps_sparse_over_tol"],
                 "us_per_stage": 1e5 * stt["wall_s"] / max(stt["steps"], 1),
-                "full_runs": "profiles/ holds the wall times of the runs to t=1e5 (config 3) and t=1e7 (config 4)"}
+                "step_kernel": ("one persistent cooperative kernel per batch of 50 steps (csrc/advance_s4.cu)"
+                                if args.step_mode == 0 else "one CUDA graph of 21 kernel nodes per step (csrc/rk_step.cu)"),
+                "full_runs": "profiles/r2_trajectories.md holds the wall times of the runs to t=1e5 (config 3) and t=1e7 (config 4)"}
 
     value = job_value(EVALS_PER_PAIR * pairs, args.steps, world, ms_total)
     line = {
@@ -492,6 +494,8 @@ def main():
     ap.add_argument("--ref-targets", type=int, default=4096, help="targets per oracle sample")
     ap.add_argument("--ref-seconds", type=float, default=10.0, help="CPU time of the oracle sample in the ours arm")
     ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--step-mode", type=int, default=0, choices=[0, 1],
+                    help="trajectory segment: 0 = persistent kernel per batch (S = 4, L <= 512), 1 = graph of launches")
     ap.add_argument("--traj-seconds", type=float, default=8.0,
                     help="wall-time budget of the adaptive trajectory segment (0 = skip)")
     ap.add_argument("--values-only", action="store_true",

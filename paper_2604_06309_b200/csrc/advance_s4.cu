@@ -335,47 +335,19 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
       }
       if (lane == 0) s_part[0][warp] = am, s_part[1][warp] = ae, s_part[2][warp] = eacc;
       __syncthreads();  // also: s_cur, s_q* complete
-      // the 16 warp sums, added in the same butterfly order by every warp of every CTA
-      double tm = s_part[0][lane & (ADV_WARPS - 1)], te = s_part[1][lane & (ADV_WARPS - 1)];
-      double eps = s_part[2][lane & (ADV_WARPS - 1)];
+      // mu (Eq.(13)) and E (Eq.(14)) from the 16 warp sums, added in a fixed order; only the threads that combine a
+      // target (and the one that writes the scalars) need them, so this is off the path to the pair loops
+      auto stage_mu = [&](double &mu, double &E) {
+        double tm = 0.0, te = 0.0;
 #pragma unroll
-      for (int o = ADV_WARPS / 2; o > 0; o >>= 1) {
-        tm += __shfl_xor_sync(0xffffffffu, tm, o);
-        te += __shfl_xor_sync(0xffffffffu, te, o);
-        eps += __shfl_xor_sync(0xffffffffu, eps, o);
-      }
-      const double c0 = s_c0;
-      double mu = mc.T + tM * tm, E = -tM * te;  // Eq.(13), Eq.(14)
-      if (mc.beta0 != 0.0) {
-        mu += mc.beta0 * f1<PD>(mc, c0) * c0;
-        E -= mc.beta0 * horner(mc.c0, mc.pmax, c0);
-      }
-      if (k == 9) {  // eps_RK (Eq.(25)) and the controller (reading G20)
-        eps_step = eps;
-        if (!a.fixed_step) {
-          if (!isfinite(eps) || eps > 2.0 * a.tol) {
-            accept = 0;
-            hn = fmin(h / 2.0, a.cap);
-          } else {
-            if (eps > a.tol)
-              hn = 0.9 * h;
-            else if (eps < a.tol / 2.0)
-              hn = 1.01 * h;
-            hn = fmin(hn, a.cap);
-          }
+        for (int w = 0; w < ADV_WARPS; ++w) tm += s_part[0][w], te += s_part[1][w];
+        const double c0 = s_c0;
+        mu = mc.T + tM * tm, E = -tM * te;
+        if (mc.beta0 != 0.0) {
+          mu += mc.beta0 * f1<PD>(mc, c0) * c0;
+          E -= mc.beta0 * horner(mc.c0, mc.pmax, c0);
         }
-      }
-      if (blockIdx.x == 0 && tid == 0) {
-        a.t[M] = tM;
-        a.scal[SC_MU] = mu;
-        a.scal[SC_E] = E;
-        if (k == 9) {
-          a.scal[SC_EPS] = eps;
-          a.scal[SC_HNEXT] = hn;
-          a.scal[SC_ACCEPT] = (double)accept;
-          a.iscal[IS_ACCEPT] = accept;
-        }
-      }
+      };
       for (int s0 = tid; s0 < L - 3; s0 += ADV_THREADS) {  // cubic forms of the row just formed
         const double2 y0 = s_cur[s0], y1 = s_cur[s0 + 1], y2 = s_cur[s0 + 2], y3 = s_cur[s0 + 3];
         s_coefM[2 * (size_t)s0] = cubic_form(y0.x, y1.x, y2.x, y3.x);
@@ -579,13 +551,20 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
           }
           // ---- top pairs (j >= jtop[i]: n2 = M - 1): rows M-1 and M through their coefficient forms, quadratic
           // in t (reading G12): B = (1 - u^2) Y_{M-1} + d (1 - u) Y'_{M-1} + u^2 Y_M ----
+          // The six cubics of a stencil start stay in registers while the start does not change (psi moves slowly
+          // over the top interval): most top pairs read nothing but the A factor's four cells.
+          int a3_held = -1;
+          double4 qc = make_double4(0, 0, 0, 0), qdc = qc, qr = qc, qdr = qc, uc = qc, ur = qc;
 #pragma unroll
           for (int q = 0; q < KMAX; ++q) {
             if (q >= Kg && q < K) {
               const int a3 = tab_start(e3[q]);
-              const double4 qc = s_coefT[4 * a3], qdc = s_coefT[4 * a3 + 1];
-              const double4 qr = s_coefT[4 * a3 + 2], qdr = s_coefT[4 * a3 + 3];
-              const double4 uc = s_coefM[2 * a3], ur = s_coefM[2 * a3 + 1];
+              if (a3 != a3_held) {
+                qc = s_coefT[4 * a3], qdc = s_coefT[4 * a3 + 1];
+                qr = s_coefT[4 * a3 + 2], qdr = s_coefT[4 * a3 + 3];
+                uc = s_coefM[2 * a3], ur = s_coefM[2 * a3 + 1];
+                a3_held = a3;
+              }
               const double v3 = tab_v(e3[q]);
               const double2 A2 = a_factor(s_cur, e2[q]);
               const double d = tau2[q] - rtT.x;
@@ -621,6 +600,8 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
             for (int w = 0; w < G; ++w) sacc += red[parity][group * G + w][q];
             Sd[q] = sacc;
           }
+          double mu, E;
+          stage_mu(mu, E);
           double b1c_first = 0.0;  // C(theta_i t, 0): the beta0 forcing of Eq.(12)
           if (mc.beta0 != 0.0) {
             const double4 lo = ld_cell(hist + (size_t)n1 * (size_t)L);
@@ -647,6 +628,37 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
               if (a.energy) a.energy[M] = E;
             }
           }
+        }
+      }
+      if (k == 9) {  // eps_RK (Eq.(25)) and the controller (reading G20), identical in every thread
+        double eps = 0.0;
+#pragma unroll
+        for (int w = 0; w < ADV_WARPS; ++w) eps += s_part[2][w];
+        eps_step = eps;
+        if (!a.fixed_step) {
+          if (!isfinite(eps) || eps > 2.0 * a.tol) {
+            accept = 0;
+            hn = fmin(h / 2.0, a.cap);
+          } else {
+            if (eps > a.tol)
+              hn = 0.9 * h;
+            else if (eps < a.tol / 2.0)
+              hn = 1.01 * h;
+            hn = fmin(hn, a.cap);
+          }
+        }
+      }
+      if (blockIdx.x == 0 && tid == 0) {
+        double mu, E;
+        stage_mu(mu, E);
+        a.t[M] = tM;
+        a.scal[SC_MU] = mu;
+        a.scal[SC_E] = E;
+        if (k == 9) {
+          a.scal[SC_EPS] = eps_step;
+          a.scal[SC_HNEXT] = hn;
+          a.scal[SC_ACCEPT] = (double)accept;
+          a.iscal[IS_ACCEPT] = accept;
         }
       }
       grid_arrive(a.bar, bar_target, nb);
