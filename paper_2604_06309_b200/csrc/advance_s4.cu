@@ -241,7 +241,8 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
         if (c == 0) s_br[0].x = n;
         if (c == L - 1) s_br[L - 4].y = n;
       }
-      __syncthreads();
+      // no CTA barrier here: jtop does not read the brackets, and a CTA barrier follows before the pair phase reads
+      // either (the one that ends grid_wait, or the one after the stage update)
       if (wg == 0) {
         for (int i = group * (int)nb + blockIdx.x; i < L; i += (int)nb * ngroups) {
           const double th_i = a.theta[i], om_i = a.omega[i];
@@ -375,6 +376,7 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
         // every phase requests what all of the thread's pairs need before it uses any of it.
         constexpr int KMAX = 4;
         double2 mw = make_double2(0.0, 0.0);  // weights of mu(theta_i t_M); used by the group's first thread
+        double mu = 0.0, E = 0.0;             // mu(t_M), E(t_M) of this stage; likewise
         const uint64_t *pt1 = a.tab + (size_t)i * (size_t)L + tig;
         const uint64_t *pt2 = pt1 + plane, *pt3 = pt2 + plane;
         // ================= type-1 half of Eq.(21): S1, S3, S5, S6 =================
@@ -600,7 +602,6 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
             for (int w = 0; w < G; ++w) sacc += red[parity][group * G + w][q];
             Sd[q] = sacc;
           }
-          double mu, E;
           stage_mu(mu, E);
           double b1c_first = 0.0;  // C(theta_i t, 0): the beta0 forcing of Eq.(12)
           if (mc.beta0 != 0.0) {
