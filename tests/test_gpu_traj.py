@@ -421,3 +421,40 @@ def test_step_modes_agree():
     for x, y in zip(a[4:], b[4:]):
         scale = np.max(np.abs(y), axis=tuple(range(1, y.ndim)), keepdims=True) if y.ndim > 1 else np.abs(y)
         assert np.all(np.abs(x - y) <= 1e-11 * scale + 1e-300)
+
+
+def test_step_modes_agree_on_a_long_history():
+    """Both implementations of dmfe_advance from the same synthetic state with many more rows than grid nodes
+    (6000 rows, L = 512: a grid cell of phi2 spans ~ 12 rows, so the row searches of the general pairs really
+    bisect): four fixed steps, new rows compared at the rounding level."""
+    import torch
+    from paper_2604_06309_b200 import dmfe as D0, inputs
+    L, s, N, n_steps, h = 512, 4, 6000, 4, 0.05
+    outs = []
+    for mode in (0, 1):
+        ctx = D0.dmfe_create(L, s, 1e4, [0, 0, 0, 1.0], T=0.5, tol=1e-8)
+        try:
+            D0.dmfe_set_step_mode(ctx, mode)
+            tab = D0.dmfe_get_tables(ctx, L)
+            t, mu, hist = inputs.random_smooth_history(tab["theta"], tab["omega"], N, 600.0, seed=11)
+            st, ten = D0.make_state(L, N + n_steps + 2)
+            ten["t"][:N] = torch.from_numpy(t).cuda()
+            ten["mu"][:N] = torch.from_numpy(mu).cuda()
+            ten["hist"][:N] = torch.from_numpy(hist).cuda()
+            st.n_rows = N
+            D0.dmfe_set_step_size(ctx, st, h)
+            res, log, rc = D0.dmfe_advance(ctx, st, n_steps, fixed_step=True, want_log=True)
+            assert res.steps == n_steps and st.n_rows == N + n_steps
+            torch.cuda.synchronize()
+            outs.append((ten["t"][N:N + n_steps].cpu().numpy(), ten["mu"][N:N + n_steps].cpu().numpy(),
+                         ten["hist"][N:N + n_steps].cpu().numpy(), log))
+        finally:
+            D0.dmfe_destroy(ctx)
+    a, b = outs
+    assert np.array_equal(a[0], b[0])
+    assert np.all(np.isfinite(a[2])) and np.all(np.isfinite(b[2]))
+    assert np.max(np.abs(a[1] - b[1]) / np.abs(b[1])) < 1e-12
+    for k in range(4):
+        scale = np.max(np.abs(b[2][:, :, k]), axis=1, keepdims=True)
+        assert np.max(np.abs(a[2][:, :, k] - b[2][:, :, k]) / scale) < 1e-10, "history component %d" % k
+    assert np.max(np.abs(a[3][:, 1] - b[3][:, 1]) / np.abs(b[3][:, 1])) < 1e-4          # eps_RK: a difference of derivatives
