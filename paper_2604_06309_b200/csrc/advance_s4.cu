@@ -157,6 +157,7 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
   __shared__ double red[2][ADV_WARPS][8];
   __shared__ double s_part[3][ADV_WARPS];
   __shared__ double s_c0;
+  __shared__ double s_mu[2];  // mu(t_M), E(t_M) of the stage
   __shared__ int s_fail;
   const int L = a.L;
   double2 *s_q1 = reinterpret_cast<double2 *>(smem_dyn), *s_q2 = s_q1 + L, *s_dl = s_q2 + L;
@@ -349,6 +350,11 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
           E -= mc.beta0 * horner(mc.c0, mc.pmax, c0);
         }
       };
+      if (warp == ADV_WARPS - 1 && lane == 0) {  // one thread; the CTA barrier below publishes it
+        double mu, E;
+        stage_mu(mu, E);
+        s_mu[0] = mu, s_mu[1] = E;
+      }
       for (int s0 = tid; s0 < L - 3; s0 += ADV_THREADS) {  // cubic forms of the row just formed
         const double2 y0 = s_cur[s0], y1 = s_cur[s0 + 1], y2 = s_cur[s0 + 2], y3 = s_cur[s0 + 3];
         s_coefM[2 * (size_t)s0] = cubic_form(y0.x, y1.x, y2.x, y3.x);
@@ -376,7 +382,6 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
         // every phase requests what all of the thread's pairs need before it uses any of it.
         constexpr int KMAX = 4;
         double2 mw = make_double2(0.0, 0.0);  // weights of mu(theta_i t_M); used by the group's first thread
-        double mu = 0.0, E = 0.0;             // mu(t_M), E(t_M) of this stage; likewise
         const uint64_t *pt1 = a.tab + (size_t)i * (size_t)L + tig;
         const uint64_t *pt2 = pt1 + plane, *pt3 = pt2 + plane;
         // ================= type-1 half of Eq.(21): S1, S3, S5, S6 =================
@@ -592,17 +597,21 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
           group_barrier(1 + group, TG);
         else
           __syncwarp();
-        if (tig == 0) {
-          // per-target combination (rhs_common.cuh: combine_target): Eq.(1), the second-argument equations
-          // (readings G9, G10) and the ray derivative of Eq.(22)
-          double Sd[8];
-#pragma unroll
-          for (int q = 0; q < 8; ++q) {
-            double sacc = 0.0;
-            for (int w = 0; w < G; ++w) sacc += red[parity][group * G + w][q];
-            Sd[q] = sacc;
+        if (wg == 0) {
+          // per-target combination (rhs_common.cuh: combine_target): Eq.(1), the second-argument equations (readings
+          // G9, G10) and the ray derivative of Eq.(22).  Lanes 0..3 of the group's first warp form d1C, d1R, d2C, d2R
+          // side by side with the same instructions: value = c X + t_M (k_a S_a + k_b S_b + k_c S_c) + add_1 + add_2
+          const int r = lane & 3;
+          const int qa = (r == 0) ? 0 : ((r == 1) ? 3 : ((r == 2) ? 4 : 7));
+          const bool three = (r == 0) || (r == 2);
+          double Sa = 0.0, Sb = 0.0, Sc = 0.0;
+          for (int w = 0; w < G; ++w) {
+            const double *rw = red[parity][group * G + w];
+            Sa += rw[qa];
+            Sb += three ? rw[qa + 1] : 0.0;
+            Sc += three ? rw[qa + 2] : 0.0;
           }
-          stage_mu(mu, E);
+          const double mu = s_mu[0], E = s_mu[1];
           double b1c_first = 0.0;  // C(theta_i t, 0): the beta0 forcing of Eq.(12)
           if (mc.beta0 != 0.0) {
             const double4 lo = ld_cell(hist + (size_t)n1 * (size_t)L);
@@ -614,19 +623,26 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
           const double2 ci = s_cur[i], cz = s_cur[0];
           const double fc = mc.beta0 * f1<PD>(mc, cz.x) * b1c_first;
           const double fc2 = mc.beta0 * f1<PD>(mc, b1c_first) * cz.x;
-          const double d1C = -mu * ci.x + tM * (th_i * Sd[0] + om_i * Sd[1] + th_i * Sd[2]) + fc;
-          const double d1R = -mu * ci.y + tM * (om_i * Sd[3]);
-          const double d2C = -mu_p * ci.x + tM * (th_i * Sd[4] + th_i * Sd[5] + om_i * Sd[6]) + 2.0 * mc.T * ci.y + fc2;
-          const double d2R = mu_p * ci.y - tM * (om_i * Sd[7]);
-          const double FC = d1C + th_i * d2C, FR = d1R + th_i * d2R;
-          Fout[i] = make_double2(FC, FR);
-          if (k == 9) {  // this evaluation completes the appended row
-            double *cell = reinterpret_cast<double *>(a.hist + (size_t)M * (size_t)L + i);
-            cell[1] = FC;
-            cell[3] = FR;
-            if (i == 0) {
-              a.mu[M] = mu;
-              if (a.energy) a.energy[M] = E;
+          // r = 0: d1C = -mu C_i + t (th S1 + om S2 + th S3) + fc          r = 1: d1R = -mu R_i + t (om S4)
+          // r = 2: d2C = -mu' C_i + t (th S5 + th S6 + om S7) + 2 T R_i + fc2    r = 3: d2R = mu' R_i - t (om S8)
+          const double cX = (r == 0) ? -mu * ci.x : ((r == 1) ? -mu * ci.y : ((r == 2) ? -mu_p * ci.x : mu_p * ci.y));
+          const double ka = (r == 0 || r == 2) ? th_i : ((r == 1) ? om_i : -om_i);
+          const double kb = (r == 0) ? om_i : ((r == 2) ? th_i : 0.0);
+          const double kc = (r == 0) ? th_i : ((r == 2) ? om_i : 0.0);
+          const double add1 = (r == 0) ? fc : ((r == 2) ? 2.0 * mc.T * ci.y : 0.0);
+          const double add2 = (r == 2) ? fc2 : 0.0;
+          const double val = cX + tM * (ka * Sa + kb * Sb + kc * Sc) + add1 + add2;
+          const double other = __shfl_down_sync(0xffffffffu, val, 2);  // lane 0: d2C, lane 1: d2R
+          const double Fv = val + th_i * other;                          // lane 0: F_C, lane 1: F_R
+          if (lane < 2) {
+            reinterpret_cast<double *>(Fout + i)[lane] = Fv;
+            if (k == 9) {  // this evaluation completes the appended row
+              double *cell = reinterpret_cast<double *>(a.hist + (size_t)M * (size_t)L + i);
+              cell[1 + 2 * lane] = Fv;
+              if (i == 0 && lane == 0) {
+                a.mu[M] = mu;
+                if (a.energy) a.energy[M] = E;
+              }
             }
           }
         }
@@ -650,11 +666,9 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
         }
       }
       if (blockIdx.x == 0 && tid == 0) {
-        double mu, E;
-        stage_mu(mu, E);
         a.t[M] = tM;
-        a.scal[SC_MU] = mu;
-        a.scal[SC_E] = E;
+        a.scal[SC_MU] = s_mu[0];
+        a.scal[SC_E] = s_mu[1];
         if (k == 9) {
           a.scal[SC_EPS] = eps_step;
           a.scal[SC_HNEXT] = hn;
