@@ -82,16 +82,20 @@ __device__ __forceinline__ unsigned long long global_ns() {
   return v;
 }
 
+// The thread that arrives and spins for its CTA sits in the last warp: the release stalls its warp for a round trip
+// to L2, and that warp is given no table work between the two halves of the barrier.
+constexpr int BAR_THREAD = ADV_THREADS - 32;
+
 // Grid barrier of the (cooperative) grid in two halves, so that work that needs nothing from the other CTAs can
 // run between them: grid_arrive publishes this CTA's writes, grid_wait returns once every CTA has arrived (false
 // when that did not happen within two seconds).
 __device__ __forceinline__ void grid_arrive(unsigned *ctr, unsigned &target, unsigned nb) {
   __syncthreads();
   target += nb;
-  if (threadIdx.x == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(ctr) : "memory");
+  if (threadIdx.x == BAR_THREAD) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(ctr) : "memory");
 }
 __device__ __forceinline__ bool grid_wait(unsigned *ctr, unsigned target, int *s_fail) {
-  if (threadIdx.x == 0) {
+  if (threadIdx.x == BAR_THREAD) {
     const unsigned long long t0 = global_ns();
     for (;;) {
       unsigned v;
@@ -224,7 +228,7 @@ __global__ void __launch_bounds__(ADV_THREADS, 1) advance_s4_kernel(AdvArgs a, M
     // (the weights of mu(theta_i t_M) are formed in the pair phase, behind the loads of the type-1 half) ----
     auto build_tables = [&](const double tM) {
       const int top = M - 1;
-      for (int c = tid; c < L; c += ADV_THREADS) {
+      for (int c = tid; c < L && tid < BAR_THREAD; c += BAR_THREAD) {  // every warp but the barrier's
         const double tau1 = __dmul_rn(a.theta[c], tM);
         const int g = min(max(s_blo[c], 0), top);
         const double ta = (g >= 1) ? a.t[g - 1] : -INFINITY, tb = a.t[g];
