@@ -43,6 +43,7 @@ static void free_all(dmfe_ctx *c) {
   cudaFree(c->cur);
   cudaFree(c->scal);
   cudaFree(c->iscal);
+  cudaFree(c->tgt_next);
   cudaFree(c->rk);
   cudaFree(c->dpk);
   cudaFree(c->eps_sp);
@@ -111,6 +112,7 @@ int dmfe_create(const dmfe_params *params, const double *lambda, double T, dmfe_
     if (e == cudaSuccess) e = cudaMalloc(&c->coefT, sizeof(double) * 16 * (size_t)L);
     if (e == cudaSuccess) e = cudaMalloc(&c->scal, sizeof(double) * SC_COUNT);
     if (e == cudaSuccess) e = cudaMalloc(&c->iscal, sizeof(int32_t) * IS_COUNT);
+    if (e == cudaSuccess) e = cudaMalloc(&c->tgt_next, sizeof(int32_t) * 32);
     if (e == cudaSuccess) e = cudaMalloc(&c->rk, sizeof(double) * 8 * (size_t)L);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_scal, sizeof(double) * SC_COUNT);
     if (e == cudaSuccess) e = cudaMallocHost(&c->h_iscal, sizeof(int32_t) * IS_COUNT);

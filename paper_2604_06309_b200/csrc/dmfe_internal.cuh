@@ -72,6 +72,7 @@ struct dmfe_ctx {
   int32_t *jtop;    // [L] first node of every target whose type-2 interval is the top one
   double *coefM;    // [L][8]  centred cubics of {C, R} of the current row, per stencil start
   double *coefT;    // [L][16] centred cubics of {C, dC, R, dR} of row M-1
+  int32_t *tgt_next;  // [1] work counter of the S = 4 pair kernel (reset by the pre-pass of every evaluation)
   int32_t rowtab_cap;
   int rowtab_dirty;  // the row table was (or may have been) rebuilt for another history: rebuild it in full
   double *scal;     // [SC_COUNT]

@@ -51,6 +51,8 @@ struct PrepS4 {
   double4 *coefM;    // [L-3][2] cubics of {C, R} of row M
   double4 *coefT;    // [L-3][4] cubics of {C, dC, R, dR} of row M-1
   const double *omega;
+  int32_t *tgt_next;   // work counter of the pair kernel: reset to the first target its groups fetch dynamically
+  int32_t tgt_first;
 };
 
 __device__ __forceinline__ double4 centred_cubic(double y0, double y1, double y2, double y3) {
@@ -224,6 +226,7 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
     sg.t[M] = tM;
     if (k == 0) scal[SC_H] = h;
   }
+  if (s4.on && threadIdx.x == 0) *s4.tgt_next = s4.tgt_first;
   if (s4.on) {  // coefficient form of the row just packed (block-wide: a start needs four neighbours)
     __syncthreads();
     const double2 *src = (L <= PREP_SCUR) ? s_cur : cur;  // small L: no round trip through L2
@@ -308,6 +311,26 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
     memset(&sg, 0, sizeof(sg));
     sg.k = -1;
   }
+  // persistent grid: one CTA per SM.  G = warps per target group.  As few as possible (long loops
+  // over j), subject to (a) every warp slot of the GPU has work (L * G >= resident warps) and (b)
+  // the number of rounds ceil(L / (groups per CTA * SMs)) wastes less than 3 % of the last round
+  // (else the best G).
+  const int warps_cta = (s4 ? S4_THREADS : RHS_THREADS) / 32;
+  int G = 1;
+  {
+    double best = -1.0;
+    for (int g = 1; g <= warps_cta && g <= 16; g *= 2) {
+      if (warps_cta % g) continue;
+      const long long slots = (long long)ctx->sm_count * (warps_cta / g);
+      const long long rounds = ((long long)L + slots - 1) / slots;
+      const double eff = (double)L / (double)(rounds * slots);
+      if (eff > best + 1e-9) best = eff, G = g;
+      if (eff >= 0.97) break;
+    }
+  }
+  const int ngroups = warps_cta / G;
+  int grid = (L + ngroups - 1) / ngroups;
+  if (grid > ctx->sm_count) grid = ctx->sm_count;
   PrepS4 ps;
   ps.on = s4 ? 1 : 0;
   ps.br = ctx->br;
@@ -315,6 +338,8 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   ps.coefM = reinterpret_cast<double4 *>(ctx->coefM);
   ps.coefT = reinterpret_cast<double4 *>(ctx->coefT);
   ps.omega = ctx->omega;
+  ps.tgt_next = ctx->tgt_next;
+  ps.tgt_first = grid * ngroups;  // the first round of targets is static (CTA b, group g: target b * ngroups + g)
   CUDA_TRY(ctx, launch_pdl(prepare_kernel, pb, PREP_THREADS, 0, ctx->stream, L, M, ctx->model, sg, ctx->theta,
                            ctx->nu, t, (const double4 *)hist, ctx->cur, ctx->rowtab, ctx->blo, ctx->scal, mu_hist,
                            ctx->muw, ps));
@@ -339,6 +364,8 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   a.coefM = reinterpret_cast<const double4 *>(ctx->coefM);
   a.coefT = reinterpret_cast<const double4 *>(ctx->coefT);
   a.scal = ctx->scal;
+  a.G = G;
+  a.tgt_next = ctx->tgt_next;
   a.deriv_row = reinterpret_cast<double4 *>(deriv_row);
   if (stage && stage->dev_rows) {
     a.dev_rows = stage->dev_rows;
@@ -360,27 +387,6 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
     }
     CUDA_TRY(ctx, cudaEventRecord(ctx->ev[2 * ctx->ev_n], ctx->stream));
   }
-  // persistent grid: one CTA per SM.  G = warps per target group.  As few as possible (long loops
-  // over j), subject to (a) every warp slot of the GPU has work (L * G >= resident warps) and (b)
-  // the number of rounds ceil(L / (groups per CTA * SMs)) wastes less than 3 % of the last round
-  // (else the best G).
-  const int warps_cta = (s4 ? S4_THREADS : RHS_THREADS) / 32;
-  int G = 1;
-  {
-    double best = -1.0;
-    for (int g = 1; g <= warps_cta && g <= 16; g *= 2) {
-      if (warps_cta % g) continue;
-      const long long slots = (long long)ctx->sm_count * (warps_cta / g);
-      const long long rounds = ((long long)L + slots - 1) / slots;
-      const double eff = (double)L / (double)(rounds * slots);
-      if (eff > best + 1e-9) best = eff, G = g;
-      if (eff >= 0.97) break;
-    }
-  }
-  a.G = G;
-  const int ngroups = warps_cta / G;
-  int grid = (L + ngroups - 1) / ngroups;
-  if (grid > ctx->sm_count) grid = ctx->sm_count;
   const int rc = s4 ? dmfe_launch_pairs_s4(ctx, a, grid) : dmfe_launch_pairs_generic(ctx, a, grid);
   if (rc != DMFE_OK) return rc;
   if (timed) {

@@ -103,6 +103,7 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
     if (SMR) rowtab = s_row;
   }
   __shared__ double red[2][S4_THREADS / 32][8];
+  __shared__ int s_base[2];  // first target of the CTA's next round
 
   const int G = a.G;
   const int TG = 32 * G;
@@ -120,7 +121,17 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
   const int K = (tig < L) ? (L - tig + TG - 1) / TG : 0;  // pairs j = tig + k TG of this thread
   int parity = 0;
 
-  for (int i = blockIdx.x * ngroups + group; i < L; i += gridDim.x * ngroups, parity ^= 1) {
+  // Rounds of ngroups adjacent targets per CTA (adjacent targets share their type-1 rows and table lines in L1).
+  // The first round of a CTA is fixed (targets b * ngroups ...); after that a CTA takes the next block of targets
+  // that nobody has taken yet from a counter in global memory (reset by the pre-pass).  Targets get cheaper with
+  // growing i (fewer general pairs), so the expensive rounds go first and the SMs finish within one cheap round of
+  // each other; a static round-robin left the average SM idle for 8 % of the kernel at L = 4096 (six or seven
+  // rounds per CTA).  The result of a target does not depend on who computes it.
+  int rnd = 0;
+  for (int base = blockIdx.x * ngroups; base < L; parity ^= 1, ++rnd) {
+    if (threadIdx.x == 0) s_base[rnd & 1] = atomicAdd(a.tgt_next, ngroups);
+    const int i = base + group;
+    if (i < L) {
     const double th_i = a.theta[i], om_i = a.omega[i];
     const double tau1 = __dmul_rn(th_i, tM);
     const int n1 = a.blo[i];
@@ -372,6 +383,9 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
       }
       combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur, M);
     }
+    }  // i < L
+    __syncthreads();
+    base = s_base[rnd & 1];
   }
 }
 

@@ -206,6 +206,7 @@ struct RhsArgs {
   const double4 *coefT;   // [L-3][4] S = 4: centred cubics of {C, dC, R, dR} of row M-1
   const double *scal;     // SC_MU, SC_E written by prepare_kernel
   int32_t G;              // warps per target group
+  int32_t *tgt_next;      // S = 4: next target to hand out (groups fetch their targets after the first round)
   double4 *deriv_row;     // optional: row of the history whose derivative slots receive F
   // device-resident step (rk_step.cu): M is read from dev_rows[0]; when `complete` is set the
   // evaluation completes the appended row M: mu_w[M], energy_w[M] and the derivative slots of hist_w[M]
