@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
     sg.t[M] = tM;
     if (k == 0) scal[SC_H] = h;
   }
-  if (s4.on && threadIdx.x == 0) *s4.tgt_next = s4.tgt_first;
+  if (threadIdx.x == 0) *s4.tgt_next = s4.tgt_first;
   if (s4.on) {  // coefficient form of the row just packed (block-wide: a start needs four neighbours)
     __syncthreads();
     const double2 *src = (L <= PREP_SCUR) ? s_cur : cur;  // small L: no round trip through L2
@@ -365,7 +365,8 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   a.coefT = reinterpret_cast<const double4 *>(ctx->coefT);
   a.scal = ctx->scal;
   a.G = G;
-  a.tgt_next = ctx->tgt_next;
+  // dynamic hand-out of rounds pays from four rounds per CTA on (a CTA barrier and an atomic per round)
+  a.tgt_next = ((L + ngroups - 1) / ngroups >= 4 * grid) ? ctx->tgt_next : nullptr;
   a.deriv_row = reinterpret_cast<double4 *>(deriv_row);
   if (stage && stage->dev_rows) {
     a.dev_rows = stage->dev_rows;

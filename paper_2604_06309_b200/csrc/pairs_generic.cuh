@@ -77,6 +77,7 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
     if (SMR) rowtab = s_row;
   }
   __shared__ double red[2][RHS_THREADS / 32][8];
+  __shared__ int s_base[2];  // first target of the CTA's next round
 
   const int G = a.G;      // warps per group (power of two, <= RHS_THREADS/32)
   const int TG = 32 * G;  // threads per group = stride of j
@@ -88,7 +89,12 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
   const double tM = a.t[M];
   int parity = 0;
 
-  for (int i = blockIdx.x * ngroups + group; i < L; i += gridDim.x * ngroups, parity ^= 1) {
+  // rounds of ngroups adjacent targets per CTA, handed out dynamically after the first one (pairs_s4.cuh)
+  int rnd = 0;
+  for (int base = blockIdx.x * ngroups; base < L; parity ^= 1, ++rnd) {
+    if (a.tgt_next && threadIdx.x == 0) s_base[rnd & 1] = atomicAdd(a.tgt_next, ngroups);
+    const int i = base + group;
+    if (i < L) {
     const uint64_t *tab1 = a.tab + (size_t)i * (size_t)L, *tab2 = tab1 + plane, *tab3 = tab2 + plane;
     const double th_i = a.theta[i], om_i = a.omega[i];
     // type-1: one row search per target, tau = theta_i t  (Eq.(19)); blo[i] is exactly that row
@@ -281,6 +287,13 @@ __global__ void __launch_bounds__(RHS_THREADS, 1) history_integrals_kernel(RhsAr
       __syncwarp();
     if (tig == 0)
       combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur, M);
+    }  // i < L
+    if (a.tgt_next) {
+      __syncthreads();
+      base = s_base[rnd & 1];
+    } else {  // few rounds per CTA: static round-robin
+      base += gridDim.x * ngroups;
+    }
   }
 }
 

@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
   // rounds per CTA).  The result of a target does not depend on who computes it.
   int rnd = 0;
   for (int base = blockIdx.x * ngroups; base < L; parity ^= 1, ++rnd) {
-    if (threadIdx.x == 0) s_base[rnd & 1] = atomicAdd(a.tgt_next, ngroups);
+    if (a.tgt_next && threadIdx.x == 0) s_base[rnd & 1] = atomicAdd(a.tgt_next, ngroups);
     const int i = base + group;
     if (i < L) {
     const double th_i = a.theta[i], om_i = a.omega[i];
@@ -384,8 +384,12 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
       combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur, M);
     }
     }  // i < L
-    __syncthreads();
-    base = s_base[rnd & 1];
+    if (a.tgt_next) {
+      __syncthreads();
+      base = s_base[rnd & 1];
+    } else {  // few rounds per CTA: static round-robin
+      base += gridDim.x * ngroups;
+    }
   }
 }
 

@@ -31,6 +31,7 @@ struct ValArgs {
   const double2 *muw;    // [L] mu(theta_c t_M) = muw.x + muw.y mu(t_M)
   const double4 *win;    // [max(M-2,1)][2]: {t_k..t_k+3}, {inverse denominators}
   const double *scal;
+  int32_t *tgt_next;     // next block of targets to hand out (reset by prepare_values_kernel)
   dmfe_rhs_out out;
 };
 
@@ -42,7 +43,7 @@ __global__ void __launch_bounds__(PV_THREADS) prepare_values_kernel(int L, int M
                                                                     const double2 *__restrict__ hist,
                                                                     double2 *__restrict__ cur, int32_t *__restrict__ blo,
                                                                     double2 *__restrict__ muw, double4 *__restrict__ win,
-                                                                    double *__restrict__ scal) {
+                                                                    double *__restrict__ scal, int32_t *tgt_next, int tgt_first) {
   __shared__ double sm[32], se[32];
   __shared__ double s_c0;
   pdl_launch_dependents();
@@ -112,6 +113,7 @@ __global__ void __launch_bounds__(PV_THREADS) prepare_values_kernel(int L, int M
     const double c0 = s_c0;
     scal[SC_MU] = mc.T + tM * tm + mc.beta0 * horner(mc.c1, mc.pmax - 1, c0) * c0;
     scal[SC_E] = -tM * te - mc.beta0 * horner(mc.c0, mc.pmax, c0);
+    *tgt_next = tgt_first;
   }
 }
 
@@ -147,6 +149,7 @@ __global__ void __launch_bounds__(VAL_THREADS, 1) history_integrals_values_kerne
     cur = s_cur, blo = s_blo;
   }
   __shared__ double red[2][VAL_THREADS / 32][8];
+  __shared__ int s_base[2];  // first target of the CTA's next round
   const int G = a.G, TG = 32 * G;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int group = warp / G, wg = warp % G;
@@ -158,7 +161,12 @@ __global__ void __launch_bounds__(VAL_THREADS, 1) history_integrals_values_kerne
   const int kmax = M + 1 - npts;
   int parity = 0;
 
-  for (int i = blockIdx.x * ngroups + group; i < L; i += gridDim.x * ngroups, parity ^= 1) {
+  // rounds of ngroups adjacent targets per CTA, handed out dynamically after the first one (pairs_s4.cuh)
+  int rnd = 0;
+  for (int base = blockIdx.x * ngroups; base < L; parity ^= 1, ++rnd) {
+    if (a.tgt_next && threadIdx.x == 0) s_base[rnd & 1] = atomicAdd(a.tgt_next, ngroups);
+    const int i = base + group;
+    if (i < L) {
     const uint64_t *tab1 = a.tab + (size_t)i * (size_t)L, *tab2 = tab1 + plane, *tab3 = tab2 + plane;
     const double th_i = a.theta[i], om_i = a.omega[i];
     // type-1: one window per target, tau = theta_i t (Eq.(19))
@@ -275,7 +283,7 @@ __global__ void __launch_bounds__(VAL_THREADS, 1) history_integrals_values_kerne
       group_barrier(1 + group, TG);
     else
       __syncwarp();
-    if (tig != 0) continue;
+    if (tig == 0) {
     double Sd[8];
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
@@ -308,6 +316,14 @@ __global__ void __launch_bounds__(VAL_THREADS, 1) history_integrals_values_kerne
       if (a.out.mu) a.out.mu[0] = mu;
       if (a.out.energy) a.out.energy[0] = a.scal[SC_E];
     }
+    }  // tig == 0
+    }  // i < L
+    if (a.tgt_next) {
+      __syncthreads();
+      base = s_base[rnd & 1];
+    } else {  // few rounds per CTA: static round-robin
+      base += gridDim.x * ngroups;
+    }
   }
 }
 
@@ -325,11 +341,26 @@ int dmfe_launch_rhs_values(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double
     CUDA_TRY(ctx, cudaMalloc(&ctx->win, sizeof(double) * 8 * (size_t)cap));
     ctx->win_cap = cap;
   }
+  const int warps_cta = VAL_THREADS / 32;
+  int G = 1;
+  {
+    double best = -1.0;
+    for (int g = 1; g <= warps_cta && g <= 16; g *= 2) {
+      const long long slots = (long long)ctx->sm_count * (warps_cta / g);
+      const long long rounds = ((long long)L + slots - 1) / slots;
+      const double eff = (double)L / (double)(rounds * slots);
+      if (eff > best + 1e-9) best = eff, G = g;
+      if (eff >= 0.97) break;
+    }
+  }
+  const int ngroups = warps_cta / G;
+  int grid = (L + ngroups - 1) / ngroups;
+  if (grid > ctx->sm_count) grid = ctx->sm_count;
   int pb = 1 + (M + L + PV_THREADS - 1) / PV_THREADS;
   if (pb > 33) pb = 33;
   CUDA_TRY(ctx, launch_pdl(prepare_values_kernel, pb, PV_THREADS, 0, ctx->stream, L, M, ctx->model, ctx->theta, ctx->nu,
                            t, mu_hist, (const double2 *)hist, ctx->cur, ctx->blo, ctx->muw,
-                           reinterpret_cast<double4 *>(ctx->win), ctx->scal));
+                           reinterpret_cast<double4 *>(ctx->win), ctx->scal, ctx->tgt_next, grid * ngroups));
   ValArgs a;
   memset(&a, 0, sizeof(a));
   a.L = L;
@@ -345,6 +376,8 @@ int dmfe_launch_rhs_values(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double
   a.muw = ctx->muw;
   a.win = reinterpret_cast<const double4 *>(ctx->win);
   a.scal = ctx->scal;
+  a.G = G;
+  a.tgt_next = ((L + ngroups - 1) / ngroups >= 4 * grid) ? ctx->tgt_next : nullptr;
   a.out = *out;
   const bool timed = ctx->timing_on && ctx->ev_n < DMFE_EV_RING;
   if (timed) {
@@ -355,22 +388,6 @@ int dmfe_launch_rhs_values(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double
     }
     CUDA_TRY(ctx, cudaEventRecord(ctx->ev[2 * ctx->ev_n], ctx->stream));
   }
-  const int warps_cta = VAL_THREADS / 32;
-  int G = 1;
-  {
-    double best = -1.0;
-    for (int g = 1; g <= warps_cta && g <= 16; g *= 2) {
-      const long long slots = (long long)ctx->sm_count * (warps_cta / g);
-      const long long rounds = ((long long)L + slots - 1) / slots;
-      const double eff = (double)L / (double)(rounds * slots);
-      if (eff > best + 1e-9) best = eff, G = g;
-      if (eff >= 0.97) break;
-    }
-  }
-  a.G = G;
-  const int ngroups = warps_cta / G;
-  int grid = (L + ngroups - 1) / ngroups;
-  if (grid > ctx->sm_count) grid = ctx->sm_count;
   const size_t smem1 = 20 * (size_t)L;
   const bool smt = smem1 <= (size_t)ctx->smem_max;
   const size_t smem = smt ? smem1 : 0;
