@@ -91,7 +91,9 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
   if (blockIdx.x > 0 || gridDim.x == 1) {
     const int nb = gridDim.x == 1 ? 1 : gridDim.x - 1;
     const int b = gridDim.x == 1 ? 0 : blockIdx.x - 1;
-    const int n_extra = s4.on ? 2 * L - 3 : 0;  // jtop [L] and coefT [L-3]
+    // jtop [L] and coefT [L-3]; a host-driven evaluation (no stage update: row M is in the history) also forms
+    // coefM [L-3] here, off block 0's path
+    const int n_extra = s4.on ? 2 * L - 3 + (k < 0 ? L - 3 : 0) : 0;
     // rows below rt0 already have their final row-table entries (device-resident steps: only the
     // entries at the end of the history change between evaluations; rk_step.cu keeps the count)
     const int rt0 = sg.dev_rows ? min(max(sg.iscal[IS_RTVALID], 0), M - 1) : 0;
@@ -149,6 +151,12 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
             lo = mid + 1;
         }
         s4.jtop[i] = lo;
+      } else if (e >= M + 3 * L - 3) {
+        const int a = e - M - 3 * L + 3;  // 0 .. L-4: cubics of {C, R} of row M (host-driven evaluation only)
+        const double4 *r = hist + (size_t)M * (size_t)L + a;
+        const double4 y0 = r[0], y1 = r[1], y2 = r[2], y3 = r[3];
+        s4.coefM[2 * (size_t)a] = centred_cubic(y0.x, y1.x, y2.x, y3.x);
+        s4.coefM[2 * (size_t)a + 1] = centred_cubic(y0.z, y1.z, y2.z, y3.z);
       } else {
         const int a = e - M - 2 * L;  // 0 .. L-4
         const double4 *r = hist + (size_t)(M - 1) * (size_t)L + a;
@@ -173,7 +181,21 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
   double eacc = 0.0, am = 0.0, ae = 0.0;
   __shared__ double s_c0;
   __shared__ double2 s_cur[PREP_SCUR];
-  for (int l = threadIdx.x; l < L; l += blockDim.x) {
+  if (k < 0) {  // host-driven evaluation: row M is read, nothing is updated; several nodes' loads in flight
+#pragma unroll 4
+    for (int l = threadIdx.x; l < L; l += blockDim.x) {
+      const double4 c = rowM[l];
+      const double2 y = make_double2(c.x, c.z);
+      cur[l] = y;
+      if (l < PREP_SCUR) s_cur[l] = y;
+      if (l == 0) s_c0 = y.x;
+      const double fp = horner(mc.c1, mc.pmax - 1, y.x), fpp = horner(mc.c2, mc.pmax - 2, y.x);
+      const double nj = nu[l];
+      am += nj * (fpp * y.y * y.x + fp * y.y);
+      ae += nj * (fp * y.y);
+    }
+  }
+  for (int l = threadIdx.x; l < L && k >= 0; l += blockDim.x) {
     double2 y;  // {C, R} of row M at node l
     if (k >= 0) {
       double2 a, b, d, Fk;
@@ -227,7 +249,7 @@ __global__ void __launch_bounds__(PREP_THREADS) prepare_kernel(int L, int M, Mod
     if (k == 0) scal[SC_H] = h;
   }
   if (threadIdx.x == 0) *s4.tgt_next = s4.tgt_first;
-  if (s4.on) {  // coefficient form of the row just packed (block-wide: a start needs four neighbours)
+  if (s4.on && k >= 0) {  // coefficient form of the row just formed (block-wide: a start needs four neighbours)
     __syncthreads();
     const double2 *src = (L <= PREP_SCUR) ? s_cur : cur;  // small L: no round trip through L2
     for (int a = threadIdx.x; a < L - 3; a += blockDim.x) {
@@ -302,7 +324,8 @@ int dmfe_launch_rhs(dmfe_ctx *ctx, int32_t M, int32_t n_cap, const double *t, co
   }
   if (!(stage && stage->dev_rows)) ctx->rowtab_dirty = 1;  // host-driven evaluation: full rebuild, here and next time
   const bool s4 = ctx->p.stencil == 4 && !ctx->p.log_r;  // the log-R option runs the generic kernel
-  int pb = 1 + (M + (s4 ? 3 : 1) * L + PREP_THREADS - 1) / PREP_THREADS;
+  const bool host_call = !(stage && stage->k >= 0);
+  int pb = 1 + (M + (s4 ? (host_call ? 4 : 3) : 1) * L + PREP_THREADS - 1) / PREP_THREADS;
   if (pb > 33) pb = 33;
   dmfe_stage sg;
   if (stage) {
