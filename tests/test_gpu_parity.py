@@ -350,3 +350,28 @@ def test_bad_arguments_are_rejected(D):
             D.dmfe_history_integrals(ctx, 1, z, z, h)              # n_rows < 2
     finally:
         D.dmfe_destroy(ctx)
+
+
+@pytest.mark.parametrize("s,values_only", [(4, False), (10, False), (4, True)])
+def test_every_target_is_computed_when_rounds_are_handed_out_dynamically(D, s, values_only):
+    """L = 4096 is past the point (four rounds of targets per CTA) from which the pair kernels take their rounds from a
+    global counter instead of a static round-robin.  Outputs start as NaN: every target must have been written, by
+    whoever took it, and two evaluations must agree bit for bit (the result of a target does not depend on which CTA
+    computed it, nor on the order).  Parity against the oracle at this size: the sampled-target tests."""
+    import torch
+    L, N = 4096, 96
+    ctx = D.dmfe_create(L, s, 1e4, [0, 0, 0.6, 1.0], T=0.5, values_only=values_only)
+    try:
+        tab = D.dmfe_get_tables(ctx, L)
+        t, mu, hist = inputs.random_smooth_history(tab["theta"], tab["omega"], N, 300.0, seed=5)
+        if values_only:
+            hist = np.ascontiguousarray(hist[:, :, [0, 2]])
+        runs = []
+        for _ in range(2):
+            g = gpu_rhs(D, ctx, L, t, mu, hist, N, want_rows=False)
+            runs.append(g)
+        for k, v in runs[0].items():
+            assert np.all(np.isfinite(v)), "%s: a target was not computed" % k
+            assert np.array_equal(v, runs[1][k]), "%s differs between two evaluations" % k
+    finally:
+        D.dmfe_destroy(ctx)
