@@ -37,7 +37,8 @@ extern "C" {
 
 #define DMFE_OK 0
 #define DMFE_EINVAL (-1)      /* bad parameter (L < 2s, t_max <= e, n_rows < 2, NULL pointer ...) */
-#define DMFE_ECUDA (-2)       /* a CUDA call failed; dmfe_last_cuda_error() has the code          */
+#define DMFE_ECUDA (-2)       /* a CUDA call failed; dmfe_last_cuda_error() has the code (0 when the
+                                 persistent step kernel gave up on its grid barrier after 2 s)     */
 #define DMFE_ECAPACITY (-3)   /* a step needs a free row: n_rows + 1 > n_cap                      */
 #define DMFE_ESTEPMIN (-4)    /* controller drove h below h_min                    */
 #define DMFE_ENONFINITE (-5)  /* eps_RK not finite and nothing left to revert                     */
