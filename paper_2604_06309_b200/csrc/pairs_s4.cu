@@ -25,10 +25,14 @@ int dmfe_launch_pairs_s4(dmfe_ctx *ctx, const RhsArgs &a, int grid) {
   } while (0)
 #define DMFE_LAUNCH_S4(PD_, SM_)                                       \
   do {                                                                 \
-    if (hooks)                                                         \
-      DMFE_LAUNCH_K((history_integrals_s4_kernel<PD_, SM_, true>));    \
-    else                                                               \
-      DMFE_LAUNCH_K((history_integrals_s4_kernel<PD_, SM_, false>));   \
+    if (hooks && a.tgt_next)                                                   \
+      DMFE_LAUNCH_K((history_integrals_s4_kernel<PD_, SM_, true, true>));      \
+    else if (hooks)                                                            \
+      DMFE_LAUNCH_K((history_integrals_s4_kernel<PD_, SM_, true, false>));     \
+    else if (a.tgt_next)                                                       \
+      DMFE_LAUNCH_K((history_integrals_s4_kernel<PD_, SM_, false, true>));     \
+    else                                                                       \
+      DMFE_LAUNCH_K((history_integrals_s4_kernel<PD_, SM_, false, false>));    \
   } while (0)
 #define DMFE_LAUNCH_S4M(PD_)   \
   do {                         \

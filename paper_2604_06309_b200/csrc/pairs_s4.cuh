@@ -78,7 +78,8 @@ __device__ __forceinline__ int probe_row(const double2 *rowtab, int lo, int hi, 
   return lo;
 }
 
-template <int PD, int SM, bool HOOKS>
+// DYN: rounds of targets after a CTA's first one come from the global counter a.tgt_next (else static round-robin)
+template <int PD, int SM, bool HOOKS, bool DYN>
 __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(RhsArgs a, ModelCoef mc) {
   // SM: 0 = per-call tables read from global memory, 1 = cur and br in shared memory, 2 = rowtab too
   constexpr bool SMT = SM >= 1, SMR = SM == 2;
@@ -129,7 +130,7 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
   // rounds per CTA).  The result of a target does not depend on who computes it.
   int rnd = 0;
   for (int base = blockIdx.x * ngroups; base < L; parity ^= 1, ++rnd) {
-    if (a.tgt_next && threadIdx.x == 0) s_base[rnd & 1] = atomicAdd(a.tgt_next, ngroups);
+    if (DYN && threadIdx.x == 0) s_base[rnd & 1] = atomicAdd(a.tgt_next, ngroups);
     const int i = base + group;
     if (i < L) {
     const double th_i = a.theta[i], om_i = a.omega[i];
@@ -384,7 +385,7 @@ __global__ void __launch_bounds__(S4_THREADS, 1) history_integrals_s4_kernel(Rhs
       combine_target<PD, SMT>(a, mc, i, n1, th_i, om_i, tM, tau1, b1c_first, red[parity], group * G, G, cur, M);
     }
     }  // i < L
-    if (a.tgt_next) {
+    if (DYN) {
       __syncthreads();
       base = s_base[rnd & 1];
     } else {  // few rounds per CTA: static round-robin
